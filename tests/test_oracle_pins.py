@@ -1,0 +1,325 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these re-types the oracle's own formula: each compares it with an analytic closed form, a textbook
+special case, an invariant, a library routine (numpy FFT) used on a different formulation, or brute force.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import lam_oracle as O
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(np.asarray(b)))
+
+
+def unit_vectors(theta, phi):
+    """Normals of the two delta functions of Eq. 2, written out by hand."""
+    e_u = np.array([math.cos(theta), math.sin(theta), 0.0])
+    e_v = np.array([math.sin(theta) * math.sin(phi), -math.cos(theta) * math.sin(phi), math.cos(phi)])
+    return e_u, e_v
+
+
+def blob_projection(c, s, A, theta, phi, h, w):
+    """Line integral of A exp(-|x-c|^2/(2s^2)) along the line of Eq. 2: the two deltas fix (x.e_u, x.e_v),
+    e_u and e_v are orthonormal, so the integral is over the third orthonormal direction and equals
+    A s sqrt(2 pi) exp(-((u-c.e_u)^2+(v-c.e_v)^2)/(2 s^2))."""
+    e_u, e_v = unit_vectors(theta, phi)
+    u = np.arange(w) - w / 2
+    v = np.arange(h) - h / 2
+    return A * s * math.sqrt(2 * math.pi) * np.exp(-((u[None, :] - c @ e_u) ** 2 + (v[:, None] - c @ e_v) ** 2) / (2 * s * s))
+
+
+# ------------------------------------------------------------------ P0: the oracle's own FFT
+@pytest.mark.parametrize("n", [2, 8, 64, 12, 30])
+@pytest.mark.parametrize("sign", [-1, 1])
+def test_fft_against_naive_dft_and_numpy(n, sign):
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    fast, slow = O.dft1d(x, sign), O.dft1d(x, sign, naive=True)
+    ref = np.fft.fft(x) if sign < 0 else np.fft.ifft(x) * n
+    assert rel(fast, ref) < 1e-13 and rel(slow, ref) < 1e-13
+
+
+# ------------------------------------------------------------------ P1: Fourier-slice identity (Eqs. 5-6)
+@pytest.mark.parametrize("phi_deg", [0.0, 20.0, 35.0])
+def test_P1_fourier_slice_of_analytic_blob(phi_deg):
+    """(1/(wh)) DFT2 of the analytic blob projection = (1/(wh)) * analytic 3-D transform of the blob,
+    A (2 pi)^{3/2} s^3 exp(-2 pi^2 s^2 |xi|^2) e^{-2 pi i c.xi}, at xi of Eq. 6.  Pins the signs of Eq. 6,
+    the sign of the transform, the centring and the 1/(wh) normalisation."""
+    h = w = 64
+    phi = math.radians(phi_deg)
+    c, s, A = np.array([3.0, -5.0, 2.0]), 2.0, 0.8
+    theta = np.array([0.3, 1.9, 4.0])
+    geom = O.Geometry(n=64, h=h, w=w, theta=theta, phi=phi, filter="none")
+    proj = np.stack([blob_projection(c, s, A, t, phi, h, w) for t in theta])
+    for i, t in enumerate(theta):
+        D = O.spectrum(geom, proj, i)
+        ku = (np.arange(w) - w // 2)[None, :] / w
+        kv = (np.arange(h) - h // 2)[:, None] / h
+        xi1 = ku * math.cos(t) + kv * math.sin(t) * math.sin(phi)      # Eq. 6
+        xi2 = ku * math.sin(t) - kv * math.cos(t) * math.sin(phi)
+        xi3 = kv * math.cos(phi) + 0 * ku
+        ana = A * (2 * math.pi) ** 1.5 * s ** 3 * np.exp(-2 * math.pi ** 2 * s * s * (xi1 ** 2 + xi2 ** 2 + xi3 ** 2)) \
+            * np.exp(-2j * math.pi * (c[0] * xi1 + c[1] * xi2 + c[2] * xi3)) / (w * h)
+        assert rel(D, ana) < 1e-7
+
+
+# ------------------------------------------------------------------ P2 / P3: adjoint = Eq. 4
+def test_P2_P3_adjoint_is_backprojection_integral():
+    """Path A without filter on band-limited blob projections equals Eq. 4:
+    sum_theta d_analytic(theta, x.e_u, x.e_v) at any voxel, and on the axis the closed form
+    N_theta A s sqrt(2 pi) exp(-x3^2 cos^2(phi)/(2 s^2)) for a centred blob."""
+    n, h, w, nth = 32, 64, 64, 48
+    phi = math.radians(20.0)
+    theta = 2 * np.pi * np.arange(nth) / nth
+    s, A = 2.5, 0.7
+    geom = O.Geometry(n=n, h=h, w=w, theta=theta, phi=phi, filter="none")
+    # P3: centred blob, column through the axis
+    proj = np.stack([blob_projection(np.zeros(3), s, A, t, phi, h, w) for t in theta])
+    col = O.fbp_nudft(geom, proj, cols=[[n // 2, n // 2]])[0]
+    x3 = np.arange(n) - n / 2
+    closed = nth * A * s * math.sqrt(2 * math.pi) * np.exp(-x3 ** 2 * math.cos(phi) ** 2 / (2 * s * s))
+    assert rel(col, closed) < 1e-8
+    # P2: off-centre blob, arbitrary voxels
+    c = np.array([4.0, -3.0, 2.0])
+    proj = np.stack([blob_projection(c, s, A, t, phi, h, w) for t in theta])
+    cols = np.array([[10, 20], [16, 16], [25, 7], [20, 13]])
+    got = O.fbp_nudft(geom, proj, cols=cols)
+    want = np.zeros_like(got)
+    for ci, (i1, i2) in enumerate(cols):
+        for i3 in range(n):
+            x = np.array([i1 - n / 2, i2 - n / 2, i3 - n / 2])
+            for t in theta:
+                e_u, e_v = unit_vectors(t, phi)
+                want[ci, i3] += A * s * math.sqrt(2 * math.pi) * math.exp(
+                    -((x @ e_u - c @ e_u) ** 2 + (x @ e_v - c @ e_v) ** 2) / (2 * s * s))
+    assert rel(got, want) < 1e-8
+
+
+# ------------------------------------------------------------------ P4: phi = 0 is tomography
+@pytest.mark.parametrize("filt,tol", [("ramp", 1e-6), ("shepp-logan", 3e-2)])
+def test_P4_tomography_limit_reproduces_blob(filt, tol):
+    """At phi = 0 Eq. 1 is the Radon transform and FBP (Eq. 3) with the textbook constant
+    f = (1/2) int_0^{2 pi} (d * ramp)(x.e_u) dtheta must return the object: pins the filter constant
+    pi/N_theta and the Ram-Lak discretisation.  (Shepp-Logan is a low-pass: percent-level only.)"""
+    n, h, w, nth = 32, 64, 64, 96
+    theta = 2 * np.pi * np.arange(nth) / nth
+    c, s, A = np.array([5.0, -3.0, 2.0]), 2.0, 0.9
+    geom = O.Geometry(n=n, h=h, w=w, theta=theta, phi=0.0, filter=filt)
+    proj = np.stack([blob_projection(c, s, A, t, 0.0, h, w) for t in theta])
+    vol = O.fbp_nudft(geom, proj)
+    x = np.arange(n) - n / 2
+    X3, X2, X1 = np.meshgrid(x, x, x, indexing="ij")
+    blob = A * np.exp(-((X1 - c[0]) ** 2 + (X2 - c[1]) ** 2 + (X3 - c[2]) ** 2) / (2 * s * s))
+    assert rel(vol, blob) < tol
+
+
+# ------------------------------------------------------------------ P5: phi > 0, missing cone
+@pytest.mark.parametrize("phi_deg", [20.0, 30.0])
+def test_P5_missing_cone_closed_form(phi_deg):
+    """By Eq. 6 the frequencies with |xi3| tan(phi) > |(xi1,xi2)| are never sampled, every other one is hit
+    twice with Jacobian |k_u| cos(phi); so FBP (Eq. 3) returns the inverse 3-D transform of
+    ghat(xi) 1[|xi3| tan(phi) < |(xi1,xi2)|].  The reference is numpy's FFT of the ANALYTIC ghat on a large
+    grid.  Pins the cos(phi) in the filter constant and the geometry at phi > 0.  (Limited by the reference's
+    own discretisation of the cone edge: 1e-3 level.)"""
+    phi = math.radians(phi_deg)
+    n, h, w, nth = 32, 64, 64, 128
+    theta = 2 * np.pi * np.arange(nth) / nth
+    c, s, A = np.array([2.0, -1.0, 1.0]), 2.0, 1.0
+    geom = O.Geometry(n=n, h=h, w=w, theta=theta, phi=phi, filter="ramp")
+    proj = np.stack([blob_projection(c, s, A, t, phi, h, w) for t in theta])
+    vol = O.fbp_nudft(geom, proj)
+    NF = 256
+    f = np.fft.fftfreq(NF)
+    F3, F2, F1 = np.meshgrid(f, f, f, indexing="ij")
+    ghat = A * (2 * math.pi) ** 1.5 * s ** 3 * np.exp(-2 * math.pi ** 2 * s * s * (F1 ** 2 + F2 ** 2 + F3 ** 2)) \
+        * np.exp(-2j * math.pi * (c[0] * F1 + c[1] * F2 + c[2] * F3))
+    rho, z = np.sqrt(F1 ** 2 + F2 ** 2), np.abs(F3) * math.tan(phi)
+    mask = (z < rho).astype(float) + 0.5 * (z == rho)
+    ref = np.fft.ifftn(ghat * mask).real          # sum_xi ghat e^{+2 pi i x xi} dxi^3, dxi = 1/NF
+    idx = (np.arange(n) - n // 2) % NF
+    ref = ref[np.ix_(idx, idx, idx)]
+    assert rel(vol, ref) < 4e-3
+    x = np.arange(n) - n / 2
+    X3, X2, X1 = np.meshgrid(x, x, x, indexing="ij")
+    blob = A * np.exp(-((X1 - c[0]) ** 2 + (X2 - c[1]) ** 2 + (X3 - c[2]) ** 2) / (2 * s * s))
+    assert rel(vol, blob) > 0.05                  # the test has teeth: the raw blob is far away
+
+
+# ------------------------------------------------------------------ P6: transposes
+def test_P6_adjoint_identity_exact_operators():
+    """<L f, d> = <f, L* d> to 1e-10 (north_star) for the NUDFT pair (Eq. 5 / Eq. 7) and the direct pair."""
+    rng = np.random.default_rng(5)
+    n, nz, h, w, nth = 8, 6, 10, 12, 5
+    theta = rng.uniform(0, 2 * np.pi, nth)
+    geom = O.Geometry(n=n, nz=nz, h=h, w=w, theta=theta, phi=math.radians(25.0), filter="none", cu=5.7, cv=5.2)
+    f = rng.standard_normal((nz, n, n))
+    d = rng.standard_normal((nth, h, w))
+    lhs = np.vdot(O.forward_nudft(geom, f), d)
+    rhs = np.vdot(f, O.fbp_nudft(geom, d))
+    assert abs(lhs - rhs) / abs(lhs) < 1e-10
+    lhs = np.vdot(O.fp_direct(geom, f), d)
+    rhs = np.vdot(f, O.fbp_direct(geom, d))
+    assert abs(lhs - rhs) / abs(lhs) < 1e-10
+
+
+def test_P6b_forward_nudft_matches_analytic_projection():
+    """Eq. 5 on a sampled band-limited blob returns its analytic line integrals (Eq. 1): pins O1 itself."""
+    n, h, w = 24, 24, 24
+    phi = math.radians(20.0)
+    theta = np.array([0.4, 2.2])
+    c, s, A = np.array([1.0, -2.0, 0.5]), 2.0, 1.0
+    x = np.arange(n) - n / 2
+    X3, X2, X1 = np.meshgrid(x, x, x, indexing="ij")
+    blob = A * np.exp(-((X1 - c[0]) ** 2 + (X2 - c[1]) ** 2 + (X3 - c[2]) ** 2) / (2 * s * s))
+    geom = O.Geometry(n=n, h=h, w=w, theta=theta, phi=phi, filter="none")
+    got = O.forward_nudft(geom, blob)
+    want = np.stack([blob_projection(c, s, A, t, phi, h, w) for t in theta])
+    assert rel(got, want) < 1e-5
+
+
+# ------------------------------------------------------------------ P7: brute force on tiny inputs
+def test_P7_brute_force_16():
+    rng = np.random.default_rng(7)
+    n, nz, h, w, nth = 16, 8, 16, 16, 6
+    theta = rng.uniform(0, 2 * np.pi, nth)
+    d = rng.standard_normal((nth, h, w))
+    for filt in ("none", "ramp"):
+        geom = O.Geometry(n=n, nz=nz, h=h, w=w, theta=theta, phi=math.radians(20.0), filter=filt, cu=8.3)
+        a = O.fbp_nudft(geom, d)
+        b = O.fbp_brute(geom, d)
+        assert rel(a, b) < 1e-12
+        cgrid = O.fbp_gridded(geom, d, kernel="kb", W=8, sigma=2.0)
+        assert rel(cgrid, a) < 1e-6      # random (non band-limited) data: high-frequency corners dominate
+
+
+def test_nonpow2_sizes_use_naive_dft():
+    rng = np.random.default_rng(8)
+    geom = O.Geometry(n=6, nz=4, h=6, w=10, theta=[0.5, 3.0], phi=0.3, filter="ramp")
+    d = rng.standard_normal((2, 6, 10))
+    assert rel(O.fbp_nudft(geom, d), O.fbp_brute(geom, d)) < 1e-12
+
+
+# ------------------------------------------------------------------ kernels of path C
+@pytest.mark.parametrize("kernel", ["kb", "gauss"])
+def test_kernel_transform_pair_by_quadrature(kernel):
+    """kaphat is the continuous Fourier transform of kap: check the closed form by numerical quadrature of
+    kap itself (Gauss: up to the truncation at |t| = W/2)."""
+    W, sigma = 6, 2.0
+    shape = O.default_shape(kernel, W, sigma)
+    t = np.linspace(-W / 2, W / 2, 20001)
+    k = np.array([O.kap(kernel, W, shape, x) for x in t])
+    for s in [0.0, 0.05, 0.125, 0.25]:
+        num = np.trapezoid(k * np.cos(2 * np.pi * s * t), t)
+        ana = O.kaphat(kernel, W, shape, s)
+        assert abs(num - ana) / ana < (1e-6 if kernel == "kb" else 2e-3)
+    assert abs(O.default_shape("kb", 6, 2.0) - 13.8551) < 1e-3
+    assert O.kap(kernel, W, shape, 0.0) == pytest.approx(1.0)
+    assert O.kap("kb", W, O.default_shape("kb", W, sigma), W / 2 + 1e-9) == 0.0
+
+
+# ------------------------------------------------------------------ P8: path C against path A
+def _tiny_case(filter="ramp", n=32, nth=24, seed=3):
+    """configs[0]-like: band-limited blobs in a thin slab, phi = 20 deg."""
+    rng = np.random.default_rng(seed)
+    h = w = n
+    phi = math.radians(20.0)
+    theta = 2 * np.pi * np.arange(nth) / nth
+    proj = np.zeros((nth, h, w))
+    for _ in range(6):
+        r, a = 0.3 * n * math.sqrt(rng.uniform()), rng.uniform(0, 2 * np.pi)
+        c = np.array([r * math.cos(a), r * math.sin(a), rng.uniform(-n / 16, n / 16)])
+        s, A = rng.uniform(1.5, 3.0), rng.uniform(0.5, 1.0)
+        proj += np.stack([blob_projection(c, s, A, t, phi, h, w) for t in theta])
+    return O.Geometry(n=n, h=h, w=w, theta=theta, phi=phi, filter=filter), proj
+
+
+def test_P8_gridded_path_matches_nudft():
+    geom, proj = _tiny_case()
+    a = O.fbp_nudft(geom, proj)
+    assert rel(O.fbp_gridded(geom, proj, kernel="kb"), a) < 1e-5          # KB, W=6, sigma=2
+    g = rel(O.fbp_gridded(geom, proj, kernel="gauss"), a)
+    assert 5e-5 < g < 2e-3                                                # reading Q5: Gaussian misses 2e-4 at W=6
+    assert rel(O.fbp_gridded(geom, proj, kernel="gauss", W=12), a) < 1e-5
+    # float32 input goes through the same path
+    assert rel(O.fbp_gridded(geom, proj.astype(np.float32)), O.fbp_nudft(geom, proj.astype(np.float32))) < 1e-5
+
+
+def test_P8b_slice_path_matches_full_gridded_and_nudft():
+    geom, proj = _tiny_case(nth=12)
+    a = O.fbp_nudft(geom, proj)
+    for i3 in (3, 16, 29):
+        sl = O.fbp_gridded_slice(geom, proj, i3)
+        rms = np.linalg.norm(a) / math.sqrt(geom.nz)             # error relative to the volume's slice RMS
+        assert np.linalg.norm(sl - a[i3]) / rms < 1e-5
+
+
+def test_Q7_out_of_band_samples_wrap():
+    """|xi1| reaches (1/2) sqrt(1+sin^2 phi) > 1/2: those samples must alias periodically (e^{2 pi i x xi} has
+    period 1 in xi on integer voxels).  A delta-like projection makes the corners matter."""
+    n = 16
+    theta = np.array([math.pi / 4, 2.0])
+    geom = O.Geometry(n=n, h=n, w=n, theta=theta, phi=math.radians(40.0), filter="none")
+    d = np.zeros((2, n, n)); d[:, n // 2 + 1, n // 2 - 2] = 1.0
+    a = O.fbp_nudft(geom, d)
+    assert rel(O.fbp_gridded(geom, d, W=10), a) < 1e-7
+
+
+# ------------------------------------------------------------------ P9: path B (sanity only)
+def test_P9_direct_path_agrees_at_percent_level():
+    geom, proj = _tiny_case()
+    a, b = O.fbp_nudft(geom, proj), O.fbp_direct(geom, proj)
+    m = slice(4, -4)
+    assert rel(b[m, m, m], a[m, m, m]) < 0.08
+
+
+# ------------------------------------------------------------------ P10: S0
+def test_P10_prep_inverts_detector_model():
+    rng = np.random.default_rng(10)
+    h, w = 8, 12
+    d = rng.uniform(0.0, 2.0, (3, h, w))
+    dark = (100 + rng.standard_normal((h, w))).astype(np.float32)
+    flat = (30000 * (1 + 0.01 * rng.standard_normal((h, w)))).astype(np.float32)
+    raw = np.exp(-d) * (flat.astype(float) - dark) + dark
+    raw16 = np.round(raw).astype(np.uint16)
+    geom = O.Geometry(n=8, h=h, w=w, theta=[0, 1, 2], phi=0.3, dark=dark, flat=flat)
+    for th in range(3):
+        got = O.prep(geom, raw16, th)
+        assert np.all(np.abs(got - d[th]) <= 0.5 / (raw[th] - dark) * 1.0001 + 1e-12)
+    z = np.zeros((3, h, w), dtype=np.uint16)                     # raw < dark: clamp at tmin
+    assert np.allclose(O.prep(geom, z, 0), -math.log(1e-6))
+
+
+# ------------------------------------------------------------------ P11: real part and Nyquist bins (reading Q8)
+def test_P11_imaginary_part_comes_from_nyquist_bins_only():
+    geom, proj = _tiny_case(n=16, nth=8)
+    re, im = O.fbp_nudft(geom, proj, return_imag=True)
+    assert 1e-5 < np.linalg.norm(im) / np.linalg.norm(re)        # a naive Hermitian shortcut would be wrong
+    # remove the Nyquist row and column of every projection spectrum -> imaginary part vanishes
+    h = w = 16
+    F = np.fft.fft2(proj, axes=(1, 2)); F[:, h // 2, :] = 0; F[:, :, w // 2] = 0
+    re2, im2 = O.fbp_nudft(geom, np.ascontiguousarray(np.fft.ifft2(F, axes=(1, 2)).real), return_imag=True)
+    assert np.linalg.norm(im2) / np.linalg.norm(re2) < 1e-13
+
+
+# ------------------------------------------------------------------ stored values (written by tests/golden/make_golden.py)
+def test_golden_nudft_tiny16_is_reproduced():
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec); spec.loader.exec_module(mg)
+    geom, d = mg.case()
+    want = np.loadtxt(os.path.join(here, "nudft_tiny16.txt")).reshape(geom.nz, geom.n, geom.n)
+    assert rel(O.fbp_nudft(geom, d), want) < 1e-13
+    assert rel(O.fbp_brute(geom, d), want) < 1e-12
+
+
+def test_paper_table1_gain_column_is_consistent():
+    """'Gain' = Linerec / Fourierrec time (the fixture is the paper's own print-out)."""
+    import os
+    t = np.loadtxt(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_table1.txt"))
+    assert np.all(np.abs(t[:, 4] / t[:, 3] - t[:, 5]) < 0.06)
