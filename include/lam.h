@@ -1,0 +1,129 @@
+/* lam.h — C ABI of the B200 (sm_100a) laminography filtered back-projection library (liblam.so).
+ *
+ * What is computed (citations are /root/reference/PAPER.md lines; readings Q1..Q16 are in DESIGN.md):
+ *
+ *   lam_backproject:  vol = W L*_phi d                                    Eq. 3
+ *                     L*_phi = F*_u3D F_2D                                Eq. 7
+ *     with the unequally spaced frequencies of Eq. 6
+ *         xi = (k_u/w) e_u(theta) + (k_v/h) e_v(theta),
+ *         e_u = (cos t, sin t, 0), e_v = (sin t sin phi, -cos t sin phi, cos phi)      Eq. 2
+ *     F*_u3D evaluated as a USFFT: convolution-type gridding with a width-W kernel onto a
+ *     grid oversampled by sigma, inverse FFT, division by the kernel transform; in the order of Eq. 9
+ *     (PAPER.md:174-179): 2-D USFFT in (x1,x2) per detector-frequency row k_v, then 1-D USFFT in x3.
+ *     In formulas:  vol[x] = Re sum_theta sum_{k_v,k_u} H[k_u] D[theta,k_v,k_u] e^{+2 pi i x.xi},
+ *         D = (1/(w h)) sum_{j_v,j_u} d[theta,j_v,j_u] e^{-2 pi i (k_u u/w + k_v v/h)},  u = j_u-c_u, v = j_v-c_v,
+ *         H = (pi cos(phi)/N_theta) DFT_w(band-limited ramp kernel)   (reading Q3 of "a suitable scaled version
+ *         of |sigma| cos(phi)"), Shepp-Logan variant, or H = 1 (pure adjoint L*).
+ *   lam_forward:      proj = L_phi vol = F*_2D F_u3D vol                   Eq. 5; the exact transpose
+ *                     of lam_backproject with filter = LAM_FILTER_NONE (adjoint test <L f, d> = <f, L* d>).
+ *   raw 16-bit input: d = -log( max( (raw-dark)/max(flat-dark,1), t_min ) ), the inverse of the detector model
+ *                     raw = e^{-d}(flat-dark)+dark of PAPER.md:99, fused into the first FFT pass.
+ *
+ * Layouts (all C-contiguous, last index fastest):
+ *   proj  [n_theta][h][w]   float32 line integrals, or uint16 raw counts (params.input = 1)
+ *   vol   [nz][n][n]        float32, voxel (i3,i2,i1) <-> x = (i1-n/2, i2-n/2, i3-nz/2)
+ *   dark, flat [h][w]       float32
+ *
+ * Pointers: proj / vol may be DEVICE pointers (in-core path; the plan's workspace must fit the device) or
+ * HOST pointers (pinned or pageable; detected with cudaPointerGetAttributes): then the library streams chunks of
+ * projections in and slabs of the volume out through its own pinned staging buffers on copy streams that overlap
+ * the compute stream (Figs. 6-7).  The caller owns proj and vol; the plan owns every workspace.
+ *
+ * All work of lam_backproject / lam_forward is enqueued on `cuda_stream` (a cudaStream_t, may be NULL = the
+ * legacy default stream) and on plan-owned streams forked from / joined to it with events; the calls return
+ * without synchronising when both pointers are device pointers.  With host pointers they return after the last
+ * copy has completed.
+ *
+ * Errors: no exception or abort crosses this boundary.  Every function returns a lam_status; lam_last_error()
+ * gives a plan-owned (or, for lam_create failures, thread-local) message.  There is NO CPU fallback: without a
+ * CUDA device every compute entry point returns LAM_ECUDA.
+ */
+#ifndef LAM_H_
+#define LAM_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lam_plan lam_plan; /* opaque; owns all device/host workspace */
+
+typedef enum {
+  LAM_OK = 0,
+  LAM_EINVAL = 1,        /* bad argument (see lam_last_error)                              */
+  LAM_ENOMEM_DEVICE = 2, /* workspace does not fit params.device_bytes / free device memory */
+  LAM_ENOMEM_HOST = 3,   /* pinned staging allocation failed                                */
+  LAM_ECUDA = 4,         /* CUDA runtime error, or no device                                */
+  LAM_EUNSUPPORTED = 5   /* valid request outside what this build implements                */
+} lam_status;
+
+enum { LAM_KERNEL_KB = 0, LAM_KERNEL_GAUSS = 1 };
+enum { LAM_FILTER_NONE = 0, LAM_FILTER_RAMP = 1, LAM_FILTER_SHEPP_LOGAN = 2 };
+enum { LAM_INPUT_F32 = 0, LAM_INPUT_U16_RAW = 1 };
+
+typedef struct {
+  int nz;              /* volume thickness in x3; 0 -> n                                                   */
+  int kernel;          /* LAM_KERNEL_KB (default) or LAM_KERNEL_GAUSS  (PAPER.md:130 names a Gaussian psi) */
+  int width;           /* W, taps per axis: 4, 6 or 8; 0 -> 6                                               */
+  float oversample;    /* sigma; 0 -> 2.0; sigma*n and sigma*nz must be powers of two                       */
+  float shape;         /* KB beta or Gaussian variance s_g^2 in grid cells; 0 -> Beatty / Dutt-Rokhlin rule */
+  int filter;          /* LAM_FILTER_*                                                                      */
+  int input;           /* LAM_INPUT_*                                                                       */
+  float center_u;      /* rotation-axis column on the detector, pixels; NaN -> w/2                          */
+  float center_v;      /* detector row hit by the ray through the origin; NaN -> h/2                        */
+  float t_min;         /* transmission clamp before -log; 0 -> 1e-6                                         */
+  size_t device_bytes; /* workspace budget; 0 -> 90 % of the free device memory at lam_create               */
+  int plane_batch;     /* k_v planes gridded + transformed per launch; 0 -> sized to stay L2-resident       */
+  int theta_chunk;     /* projections per filter/FFT launch (and per host->device copy); 0 -> auto          */
+} lam_params;
+
+/* Fill *p with the defaults (KB, W = 6, sigma = 2, ramp filter, fp32 input, centred axis). */
+void lam_default_params(lam_params* p);
+
+/* Build a plan.  n: lateral volume size (n x n x nz voxels); h, w: detector rows, columns; n_theta angles
+ * theta_rad[] (HOST pointer, copied; any values, quadrature weight 2 pi/n_theta as for a uniform full circle,
+ * PAPER.md:154-156); phi_rad: tilt of the rotation axis, 0 <= phi < pi/2, phi = 0 is tomography (Eq. 2).
+ * Requirements: n, nz, h, w even; w, h, sigma*n, sigma*nz powers of two in [32, 8192]; sigma*n >= 64.
+ * Allocates all tables and the gridding work lists (they depend on geometry only).  *out is NULL on error. */
+lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const float* theta_rad,
+                      const lam_params* p, lam_plan** out);
+
+/* dark, flat: h*w float32 each, host or device pointers, copied into the plan.  Needed before lam_backproject
+ * when params.input == LAM_INPUT_U16_RAW. */
+lam_status lam_set_darkflat(lam_plan* plan, const float* dark, const float* flat);
+
+/* vol <- W L* proj (overwrites vol).  proj: float32 or uint16 per params.input.  See the header comment for
+ * pointer kinds and stream semantics. */
+lam_status lam_backproject(lam_plan* plan, const void* proj, float* vol, void* cuda_stream);
+
+/* proj <- L vol (overwrites proj, float32), the transpose of lam_backproject with filter none (the plan's filter
+ * setting is ignored).  Device pointers only.  Not tuned: it exists for the adjoint identity. */
+lam_status lam_forward(lam_plan* plan, const float* vol, float* proj, void* cuda_stream);
+
+/* Per-stage device times of the LAST lam_backproject, milliseconds, measured with CUDA events on the plan's
+ * streams when profiling is on (lam_set_profiling(plan, 1); it adds event records but no synchronisation inside
+ * the call; this function synchronises).  ms[0] prep + filter + 2-D FFT (S0+S1), ms[1] gridding in (xi1,xi2)
+ * (S2), ms[2] inverse FFT passes in x1 and x2 (S3), ms[3] fused x3 stage: gridding in xi3 + inverse FFT +
+ * deapodise/crop/real part (S2 z-part + S3 + S4), ms[4] host<->device copies (host-pointer path), ms[5] whole call. */
+lam_status lam_stage_ms(lam_plan* plan, float ms[6]);
+lam_status lam_set_profiling(lam_plan* plan, int on);
+
+/* Workspace facts of a plan, for benchmarks and tests:
+ * info[0] device bytes allocated, info[1] k_v planes, info[2] plane batch, info[3] gridding work items (jobs),
+ * info[4] 1 if the plan streams through the host (out-of-core), info[5] theta chunk,
+ * info[6] kernel launches of the last lam_backproject, info[7] pinned host bytes. */
+lam_status lam_plan_info(const lam_plan* plan, long long info[8]);
+
+/* Message of the last error on this plan (plan == NULL: of the last failed lam_create on this thread). */
+const char* lam_last_error(const lam_plan* plan);
+
+void lam_destroy(lam_plan* plan);
+
+/* Library version string, e.g. "lam-b200 0.1 (sm_100a)". */
+const char* lam_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LAM_H_ */

@@ -1,0 +1,582 @@
+// lam_kernels.cuh — sm_100a kernels of the laminographic back-projection (see include/lam.h for the operator).
+//
+// Stage map (S-numbers are SURVEY.md §8(a) rows):
+//   k_rows     S0+S1  -log prep, row FFT along u of two real rows per complex transform, filter H[k_u] (Eq. 3)
+//   k_cols     S1     column FFT along v, Hermitian fold onto the k_v >= 0 planes, centring phases
+//   k_jobs_*   S2     work-list builder: which (tile, theta-range) pairs of a k_v plane hold samples (geometry only)
+//   k_spread   S2     gridding in (xi1, xi2): width-W kernel scatter of every sample of Eq. 6 onto its plane
+//   k_ifft_x1  S3     inverse FFT along xi1 -> x1, cropped to the n central outputs
+//   k_ifft_x2  S3     inverse FFT along xi2 -> x2, cropped
+//   k_zstage   S2+S3+S4  gridding in xi3 (depends on k_v only, Eq. 6), inverse FFT to x3, crop, real part,
+//                     division by the kernel transform on all three axes
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "fft_smem.cuh"
+#include "lam_math.h"
+
+namespace lam {
+
+constexpr int kTile = 32;               // gridding tile edge (fine-grid cells)
+constexpr int kTilePitch = kTile + 1;   // float2 elements per tile row in shared memory
+constexpr int kSpreadWarps = 8;         // warps (= private tiles) per k_spread block
+constexpr int kJobSegs = 32;            // target segments (theta crossings) per job
+constexpr int kJobMaxSpan = 1023;       // max theta span of one job (10 bits)
+constexpr int kMaxW = 8;
+
+// ---------------------------------------------------------------------------------------------------------------
+// S0 + S1a: rows
+// ---------------------------------------------------------------------------------------------------------------
+struct RowsArgs {
+  const void* proj;     // chunk base: [nth][h][w] float or uint16
+  const float* dark;    // [h][w]
+  const float* flat;
+  float tmin;
+  float2* R;            // [nth][h][WR]  filtered half spectra of the rows
+  const float2* Pu;     // [w/2+1]  H[k] e^{2 pi i k c_u / w} / (w h)
+  const float2* tw;     // twiddles of length w
+  int h, WR, nb;        // nb: row pairs per block
+};
+
+template <int LOGW, bool RAW>
+__global__ void __launch_bounds__(256) k_rows(RowsArgs a) {
+  constexpr int w = 1 << LOGW, P = fft_pitch(w);
+  extern __shared__ float2 sm[];
+  const int th = blockIdx.y, pair0 = blockIdx.x * a.nb;
+  const size_t pbase = (size_t)th * a.h * w;
+  for (int idx = threadIdx.x; idx < a.nb << LOGW; idx += blockDim.x) {
+    int t = idx >> LOGW, ju = idx & (w - 1), jv = 2 * (pair0 + t);
+    float x0, x1;
+    if (RAW) {
+      const uint16_t* p = (const uint16_t*)a.proj + pbase + (size_t)jv * w + ju;
+      float r0 = (float)p[0], r1 = (float)p[w];
+      float d0 = a.dark[jv * w + ju], d1 = a.dark[(jv + 1) * w + ju];
+      float f0 = a.flat[jv * w + ju], f1 = a.flat[(jv + 1) * w + ju];
+      float t0 = (r0 - d0) / fmaxf(f0 - d0, 1.0f), t1 = (r1 - d1) / fmaxf(f1 - d1, 1.0f);
+      x0 = -logf(fmaxf(t0, a.tmin));
+      x1 = -logf(fmaxf(t1, a.tmin));
+    } else {
+      const float* p = (const float*)a.proj + pbase + (size_t)jv * w + ju;
+      x0 = p[0];
+      x1 = p[w];
+    }
+    sm[t * P + fft_phys(ju)] = make_float2(x0, x1);
+  }
+  __syncthreads();
+  block_fft<LOGW, -1>(sm, a.nb, P, a.tw);
+  constexpr int NK = w / 2 + 1;
+  for (int idx = threadIdx.x; idx < a.nb * NK; idx += blockDim.x) {
+    int t = idx / NK, k = idx - t * NK, jv = 2 * (pair0 + t);
+    float2 zk = sm[t * P + fft_phys(fft_pos<LOGW>(k))];
+    float2 zn = sm[t * P + fft_phys(fft_pos<LOGW>((w - k) & (w - 1)))];
+    float2 ra = make_float2(0.5f * (zk.x + zn.x), 0.5f * (zk.y - zn.y));   // spectrum of the even row
+    float2 rb = make_float2(0.5f * (zk.y + zn.y), -0.5f * (zk.x - zn.x));  // spectrum of the odd row
+    float2 pu = a.Pu[k];
+    size_t o = ((size_t)th * a.h + jv) * a.WR + k;
+    a.R[o] = cmul(ra, pu);
+    a.R[o + a.WR] = cmul(rb, pu);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// S1b: columns.  Output planes S[p][theta][q], p = 0..h/2 (k_v = p, p = h/2 stands for k_v = -h/2),
+// q = 0..w (k_u = q - w/2; q = w is the +w/2 copy of the Nyquist column, reading Q8).
+// ---------------------------------------------------------------------------------------------------------------
+struct ColsArgs {
+  const float2* R;   // [nth][h][WR]
+  float2* S;         // [h/2+1][ntheta][WQ]
+  const float2* Pv;  // [h/2+1]  e^{2 pi i k_v c_v / h}
+  const float2* tw;  // length h
+  int w, WR, WQ, ntheta, th0, cb;
+};
+
+template <int LOGH>
+__global__ void __launch_bounds__(256) k_cols(ColsArgs a) {
+  constexpr int h = 1 << LOGH, P = fft_pitch(h);
+  extern __shared__ float2 sm[];
+  const int thl = blockIdx.y, k0 = blockIdx.x * a.cb;
+  const int nc = min(a.cb, a.w / 2 + 1 - k0);
+  const float2* Rb = a.R + (size_t)thl * h * a.WR + k0;
+  for (int idx = threadIdx.x; idx < h * a.cb; idx += blockDim.x) {
+    int jv = idx / a.cb, c = idx - jv * a.cb;
+    float2 v = c < nc ? Rb[(size_t)jv * a.WR + c] : make_float2(0.f, 0.f);
+    sm[c * P + fft_phys(jv)] = v;
+  }
+  __syncthreads();
+  block_fft<LOGH, -1>(sm, a.cb, P, a.tw);
+  const int hw = a.w / 2, th = a.th0 + thl;
+  for (int idx = threadIdx.x; idx < (h / 2 + 1) * a.cb; idx += blockDim.x) {
+    int p = idx / a.cb, c = idx - p * a.cb;
+    if (c >= nc) continue;
+    int k = k0 + c;
+    float2 cp = sm[c * P + fft_phys(fft_pos<LOGH>(p))];
+    float2 cm = sm[c * P + fft_phys(fft_pos<LOGH>((h - p) & (h - 1)))];
+    cm.y = -cm.y;
+    float2 pv = a.Pv[p];
+    bool mid = p > 0 && p < h / 2;
+    float wplus = mid ? (k < hw ? 2.f : 1.f) : (k < hw ? 1.f : 0.f);
+    float wminus = mid ? (k < hw ? 2.f : 1.f) : 1.f;
+    float2* Srow = a.S + ((size_t)p * a.ntheta + th) * a.WQ;
+    float2 vp = cmul(cp, pv), vm = cmul(cm, pv);
+    Srow[hw + k] = make_float2(vp.x * wplus, vp.y * wplus);
+    if (k > 0) Srow[hw - k] = make_float2(vm.x * wminus, vm.y * wminus);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// S2: gridding in (xi1, xi2).  Plane p (k_v fixed): sample (theta, k_u) sits at fine-grid position
+//   t = a1 k_u (cos t, sin t) + rho (sin t, -cos t),  a1 = M/w,  rho = M k_v sin(phi)/h      (Eq. 6 times M)
+// i.e. on a straight line per theta, tangent to the circle of radius rho.  The plane is cut into 32x32 tiles; a
+// job = (tile, theta-range); a warp owns a private shared-memory tile, walks the theta-range, clips every line
+// against the tile (+ kernel halo, + periodic images, reading Q7), and lets lane i deposit sample k_a + i.
+// ---------------------------------------------------------------------------------------------------------------
+struct SpreadGeom {
+  const double2* cs;   // [ntheta] (cos, sin) in double
+  double rho_unit;     // M sin(phi) / h
+  float a1;            // M / w
+  int M, nt, ntheta, w, hh /* h/2 */, kstride;
+};
+
+struct KerPoly {
+  float E[kMaxW / 2][kPolyHalf];
+  float O[kMaxW / 2][kPolyHalf];
+};
+
+// job word layout: x = tx[0:9) ty[9:18) th0[18:32);  y = nth[0:10) mx[10:13) my[13:16) flags[16:18) p[18:31)
+constexpr unsigned kJobExclusive = 1u, kJobFirstMulti = 2u;
+
+__device__ __forceinline__ uint2 job_pack(int tx, int ty, int th0, int nth, int mx, int my, unsigned fl, int p) {
+  return make_uint2((unsigned)tx | ((unsigned)ty << 9) | ((unsigned)th0 << 18),
+                    (unsigned)nth | ((unsigned)mx << 10) | ((unsigned)my << 13) | (fl << 16) | ((unsigned)p << 18));
+}
+
+// ku range [ka, kb] of the samples of one line whose kernel footprint can reach the tile.
+// (ox, oy): line origin relative to the tile's first cell; the sample k sits at (ox, oy) + a1 k (c, s).
+// Footprint test is conservative (margin 0.02 cells >> fp32 error of ox, oy); exact clipping is per tap.
+template <int W>
+__device__ __forceinline__ void clip_line(float ox, float oy, float c, float s, float a1, int hw, int& ka, int& kb) {
+  const float xl = -0.5f * W - 0.02f, xh = (float)(kTile - 1) + 0.5f * W + 0.02f;
+  float lo = -a1 * hw, hi = a1 * hw;
+  bool empty = false;
+  if (fabsf(c) > 1e-6f) {
+    float r = 1.0f / c, u0 = (xl - ox) * r, u1 = (xh - ox) * r;
+    lo = fmaxf(lo, fminf(u0, u1));
+    hi = fminf(hi, fmaxf(u0, u1));
+  } else if (ox < xl || ox > xh) empty = true;
+  if (fabsf(s) > 1e-6f) {
+    float r = 1.0f / s, u0 = (xl - oy) * r, u1 = (xh - oy) * r;
+    lo = fmaxf(lo, fminf(u0, u1));
+    hi = fminf(hi, fmaxf(u0, u1));
+  } else if (oy < xl || oy > xh) empty = true;
+  float ia = 1.0f / a1;
+  ka = max(-hw, (int)ceilf(lo * ia - 1e-3f));
+  kb = min(hw, (int)floorf(hi * ia + 1e-3f));
+  if (empty) { ka = 1; kb = 0; }
+}
+
+// which periodic images (shifts of -M, 0, +M per axis) of the sample cloud can reach the tile: bit sx+1 / sy+1
+__device__ __forceinline__ void image_candidates(const SpreadGeom& g, double rho, int mx0, int my0, int W, int& candx,
+                                                 int& candy) {
+  float rmax = sqrtf((float)(0.25 * (double)g.M * g.M + rho * rho)) + 0.5f * W + 1.0f;
+  candx = 0;
+  candy = 0;
+  for (int s = -1; s <= 1; ++s) {
+    // the image shifted by s*M covers [s*M - rmax, s*M + rmax]; the tile covers [m0, m0 + 31]
+    float lo = s * (float)g.M - rmax, hi = s * (float)g.M + rmax;
+    if (hi >= mx0 && lo <= mx0 + kTile - 1) candx |= 1 << (s + 1);
+    if (hi >= my0 && lo <= my0 + kTile - 1) candy |= 1 << (s + 1);
+  }
+}
+
+struct JobsArgs {
+  SpreadGeom g;
+  int p0, np;            // planes [p0, p0+np)
+  unsigned* count;       // [np][nt*nt]
+  const unsigned* off;   // [np][nt*nt] exclusive offsets within the chunk's job array (fill pass)
+  uint2* jobs;           // chunk job array (fill pass)
+};
+
+// FILL = false: count jobs per tile; FILL = true: write them.  One thread per (plane, tile).
+template <int W, bool FILL>
+__global__ void k_jobs(JobsArgs a) {
+  const SpreadGeom& g = a.g;
+  const int ntiles = g.nt * g.nt;
+  long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= (long long)a.np * ntiles) return;
+  const int pl = (int)(gid / ntiles), tile = (int)(gid - (long long)pl * ntiles);
+  const int p = a.p0 + pl, ty = tile / g.nt, tx = tile - ty * g.nt;
+  const int kv = p == g.hh ? -g.hh : p;
+  const double rho = g.rho_unit * kv;
+  const int mx0 = tx * kTile - g.M / 2, my0 = ty * kTile - g.M / 2;
+  int candx, candy;
+  image_candidates(g, rho, mx0, my0, W, candx, candy);
+  // pass A: which images are ever hit (so that all jobs of the tile carry the same masks)
+  int usex = 0, usey = 0;
+  for (int th = 0; th < g.ntheta; ++th) {
+    double2 cs = g.cs[th];
+    float c = (float)cs.x, s = (float)cs.y;
+    for (int sy = -1; sy <= 1; ++sy) {
+      if (!(candy >> (sy + 1) & 1)) continue;
+      float oy = (float)(-rho * cs.x - my0 + (double)sy * g.M);
+      for (int sx = -1; sx <= 1; ++sx) {
+        if (!(candx >> (sx + 1) & 1)) continue;
+        float ox = (float)(rho * cs.y - mx0 + (double)sx * g.M);
+        int ka, kb;
+        clip_line<W>(ox, oy, c, s, g.a1, g.w / 2, ka, kb);
+        if (ka <= kb) { usex |= 1 << (sx + 1); usey |= 1 << (sy + 1); }
+      }
+    }
+  }
+  // pass B: emit jobs
+  unsigned njobs = 0;
+  int start = -1, last = -1, cnt = 0;
+  uint2* out = FILL ? a.jobs + a.off[gid] : nullptr;
+  const unsigned total = FILL ? a.count[gid] : 0;
+  auto emit = [&](int t0, int t1) {
+    if (FILL) {
+      unsigned fl = total == 1 ? kJobExclusive : (njobs == 0 ? kJobFirstMulti : 0u);
+      out[njobs] = job_pack(tx, ty, t0, t1 - t0, usex, usey, fl, p);
+    }
+    ++njobs;
+  };
+  if (usex && usey) {
+    for (int th = 0; th < g.ntheta; ++th) {
+      double2 cs = g.cs[th];
+      float c = (float)cs.x, s = (float)cs.y;
+      bool hit = false;
+      for (int sy = -1; sy <= 1 && !hit; ++sy) {
+        if (!(usey >> (sy + 1) & 1)) continue;
+        float oy = (float)(-rho * cs.x - my0 + (double)sy * g.M);
+        for (int sx = -1; sx <= 1 && !hit; ++sx) {
+          if (!(usex >> (sx + 1) & 1)) continue;
+          float ox = (float)(rho * cs.y - mx0 + (double)sx * g.M);
+          int ka, kb;
+          clip_line<W>(ox, oy, c, s, g.a1, g.w / 2, ka, kb);
+          hit = ka <= kb;
+        }
+      }
+      if (hit) {
+        if (start < 0) start = th;
+        ++cnt;
+        last = th;
+        if (cnt == kJobSegs || th + 1 - start >= kJobMaxSpan) { emit(start, th + 1); start = -1; cnt = 0; }
+      } else if (start >= 0 && th - last > 32) {
+        emit(start, last + 1);
+        start = -1;
+        cnt = 0;
+      }
+    }
+    if (start >= 0) emit(start, last + 1);
+  }
+  if (njobs == 0) emit(0, 0);  // untouched tile: one exclusive job that stores zeros
+  if (!FILL) a.count[gid] = njobs;
+}
+
+__device__ __forceinline__ float2 lds_v(unsigned addr) {
+  float2 r;
+  asm volatile("ld.volatile.shared.v2.f32 {%0,%1}, [%2];" : "=f"(r.x), "=f"(r.y) : "r"(addr) : "memory");
+  return r;
+}
+__device__ __forceinline__ void sts_v(unsigned addr, float2 v) {
+  asm volatile("st.volatile.shared.v2.f32 [%0], {%1,%2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
+}
+
+template <int W>
+__device__ __forceinline__ void kernel_weights(const KerPoly& kp, float d, float (&wt)[W]) {
+  float d2 = d * d;
+#pragma unroll
+  for (int j = 0; j < W / 2; ++j) {
+    float e = kp.E[j][3], o = kp.O[j][3];
+#pragma unroll
+    for (int q = 2; q >= 0; --q) {
+      e = fmaf(e, d2, kp.E[j][q]);
+      o = fmaf(o, d2, kp.O[j][q]);
+    }
+    wt[j] = fmaf(d, o, e);
+    wt[W - 1 - j] = fmaf(-d, o, e);
+  }
+}
+
+struct SpreadArgs {
+  SpreadGeom g;
+  KerPoly kp;
+  const uint2* jobs;   // jobs of this launch
+  long long njobs;
+  const float2* S;     // [h/2+1][ntheta][WQ]
+  int WQ;
+  float2* G;           // [planes in batch][M][M]
+  int p0;              // first plane of the batch
+};
+
+// zero the tiles that receive atomic adds from several jobs
+__global__ void k_zero_tiles(SpreadArgs a) {
+  const int lane = threadIdx.x & 31;
+  long long j = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (j >= a.njobs) return;
+  uint2 jb = a.jobs[j];
+  if (!((jb.y >> 16) & kJobFirstMulti)) return;
+  int tx = jb.x & 0x1ff, ty = (jb.x >> 9) & 0x1ff, p = (jb.y >> 18) & 0x1fff;
+  float2* Gp = a.G + (size_t)(p - a.p0) * a.g.M * a.g.M + (size_t)(ty * kTile) * a.g.M + tx * kTile;
+  for (int r = 0; r < kTile; ++r) Gp[(size_t)r * a.g.M + lane] = make_float2(0.f, 0.f);
+}
+
+template <int W>
+__global__ void __launch_bounds__(kSpreadWarps * 32) k_spread(SpreadArgs a) {
+  extern __shared__ float2 sm[];
+  const SpreadGeom& g = a.g;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long jid = (long long)blockIdx.x * kSpreadWarps + warp;
+  if (jid >= a.njobs) return;  // no block-level barrier is used below
+  float2* tile = sm + warp * (kTile * kTilePitch);
+  const unsigned tile_addr = (unsigned)__cvta_generic_to_shared(tile);
+  const uint2 jb = a.jobs[jid];
+  const int tx = jb.x & 0x1ff, ty = (jb.x >> 9) & 0x1ff, th0 = jb.x >> 18;
+  const int nth = jb.y & 0x3ff, usex = (jb.y >> 10) & 7, usey = (jb.y >> 13) & 7;
+  const unsigned flags = (jb.y >> 16) & 3u;
+  const int p = (jb.y >> 18) & 0x1fff;
+  const int kv = p == g.hh ? -g.hh : p;
+  const double rho = g.rho_unit * kv;
+  const int mx0 = tx * kTile - g.M / 2, my0 = ty * kTile - g.M / 2;
+  const int hw = g.w / 2;
+
+  for (int i = lane; i < kTile * kTilePitch; i += 32) tile[i] = make_float2(0.f, 0.f);
+  __syncwarp();
+
+  const float2* Sp = a.S + (size_t)p * g.ntheta * a.WQ;
+  for (int tb = th0; tb < th0 + nth; tb += 32) {
+    const int th = tb + lane;
+    const bool tvalid = th < th0 + nth;
+    double2 cs = tvalid ? g.cs[th] : make_double2(1.0, 0.0);
+    const float c = (float)cs.x, s = (float)cs.y;
+    for (int sy = -1; sy <= 1; ++sy) {
+      if (!(usey >> (sy + 1) & 1)) continue;
+      const double oyd = -rho * cs.x - my0 + (double)sy * g.M;
+      for (int sx = -1; sx <= 1; ++sx) {
+        if (!(usex >> (sx + 1) & 1)) continue;
+        const double oxd = rho * cs.y - mx0 + (double)sx * g.M;
+        int ka = 1, kb = 0;
+        if (tvalid) clip_line<W>((float)oxd, (float)oyd, c, s, g.a1, hw, ka, kb);
+        // position of sample ka relative to the tile, in double (large terms cancel), then fp32
+        const double u0 = (double)g.a1 * ka;
+        const float p0x = (float)(oxd + u0 * cs.x), p0y = (float)(oyd + u0 * cs.y);
+        unsigned mask = __ballot_sync(0xffffffffu, ka <= kb);
+        while (mask) {
+          const int src = __ffs(mask) - 1;
+          mask &= mask - 1;
+          const int ska = __shfl_sync(0xffffffffu, ka, src), skb = __shfl_sync(0xffffffffu, kb, src);
+          const float sc = __shfl_sync(0xffffffffu, c, src), ss = __shfl_sync(0xffffffffu, s, src);
+          const float sx0 = __shfl_sync(0xffffffffu, p0x, src), sy0 = __shfl_sync(0xffffffffu, p0y, src);
+          const float2* Srow = Sp + (size_t)(tb + src) * a.WQ + hw;
+          const bool xdom = fabsf(sc) >= fabsf(ss);
+          // lanes take samples ska + sub + kstride*i so that two lanes never share a tap cell in one instruction
+          for (int sub = 0; sub < g.kstride; ++sub) {
+            for (int kbase = ska + sub; kbase <= skb; kbase += 32 * g.kstride) {
+              const int ku = kbase + lane * g.kstride;
+              const bool act = ku <= skb;
+              float2 v = act ? __ldg(&Srow[ku]) : make_float2(0.f, 0.f);
+              const float du = g.a1 * (float)(ku - ska);
+              const float t1 = fmaf(du, sc, sx0), t2 = fmaf(du, ss, sy0);
+              const float c1 = ceilf(t1 - 0.5f * W), c2 = ceilf(t2 - 0.5f * W);
+              const int col0 = (int)c1, row0 = (int)c2;
+              float w1[W], w2[W];
+              kernel_weights<W>(a.kp, t1 - c1 - (0.5f * W - 0.5f), w1);
+              kernel_weights<W>(a.kp, t2 - c2 - (0.5f * W - 0.5f), w2);
+              if (xdom) {
+#pragma unroll
+                for (int j1 = 0; j1 < W; ++j1) {
+                  const int col = col0 + j1;
+                  const bool okc = act && (unsigned)col < (unsigned)kTile;
+                  const float2 vw = make_float2(v.x * w1[j1], v.y * w1[j1]);
+                  float2 acc[W];
+                  bool ok[W];
+                  unsigned ad[W];
+#pragma unroll
+                  for (int j2 = 0; j2 < W; ++j2) {
+                    const int row = row0 + j2;
+                    ok[j2] = okc && (unsigned)row < (unsigned)kTile;
+                    ad[j2] = tile_addr + (unsigned)(row * kTilePitch + col) * 8u;
+                    if (ok[j2]) acc[j2] = lds_v(ad[j2]);
+                  }
+#pragma unroll
+                  for (int j2 = 0; j2 < W; ++j2) {
+                    acc[j2].x = fmaf(vw.x, w2[j2], acc[j2].x);
+                    acc[j2].y = fmaf(vw.y, w2[j2], acc[j2].y);
+                  }
+#pragma unroll
+                  for (int j2 = 0; j2 < W; ++j2)
+                    if (ok[j2]) sts_v(ad[j2], acc[j2]);
+                }
+              } else {
+#pragma unroll
+                for (int j2 = 0; j2 < W; ++j2) {
+                  const int row = row0 + j2;
+                  const bool okr = act && (unsigned)row < (unsigned)kTile;
+                  const float2 vw = make_float2(v.x * w2[j2], v.y * w2[j2]);
+                  float2 acc[W];
+                  bool ok[W];
+                  unsigned ad[W];
+#pragma unroll
+                  for (int j1 = 0; j1 < W; ++j1) {
+                    const int col = col0 + j1;
+                    ok[j1] = okr && (unsigned)col < (unsigned)kTile;
+                    ad[j1] = tile_addr + (unsigned)(row * kTilePitch + col) * 8u;
+                    if (ok[j1]) acc[j1] = lds_v(ad[j1]);
+                  }
+#pragma unroll
+                  for (int j1 = 0; j1 < W; ++j1) {
+                    acc[j1].x = fmaf(vw.x, w1[j1], acc[j1].x);
+                    acc[j1].y = fmaf(vw.y, w1[j1], acc[j1].y);
+                  }
+#pragma unroll
+                  for (int j1 = 0; j1 < W; ++j1)
+                    if (ok[j1]) sts_v(ad[j1], acc[j1]);
+                }
+              }
+            }
+          }
+        }
+      }
+    }
+  }
+  __syncwarp();
+  float2* Gp = a.G + (size_t)(p - a.p0) * g.M * g.M + (size_t)(ty * kTile) * g.M + tx * kTile;
+  if (flags & kJobExclusive) {
+    for (int r = 0; r < kTile; ++r) Gp[(size_t)r * g.M + lane] = lds_v(tile_addr + (unsigned)(r * kTilePitch + lane) * 8u);
+  } else {
+    for (int r = 0; r < kTile; ++r) {
+      float2 v = lds_v(tile_addr + (unsigned)(r * kTilePitch + lane) * 8u);
+      if (v.x != 0.f || v.y != 0.f) atomicAdd(&Gp[(size_t)r * g.M + lane], v);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// S3: inverse FFT along xi1 (rows of a plane, contiguous), cropped to the n central x1.
+//   T[pl][i2][ix] = (-1)^x sum_i G[pl][i2][i] e^{+2 pi i x i / M},  x = ix - n/2  (grid index i = m + M/2)
+// ---------------------------------------------------------------------------------------------------------------
+struct IfftArgs {
+  const float2* in;
+  float2* out;
+  const float2* tw;
+  int n, nb;  // nb: rows (x1 pass) or columns (x2 pass) per block
+};
+
+template <int LOGM>
+__global__ void __launch_bounds__(256) k_ifft_x1(IfftArgs a) {
+  constexpr int M = 1 << LOGM, P = fft_pitch(M);
+  extern __shared__ float2 sm[];
+  const int pl = blockIdx.y, r0 = blockIdx.x * a.nb;
+  const float2* in = a.in + ((size_t)pl * M + r0) * M;
+  for (int idx = threadIdx.x; idx < a.nb << LOGM; idx += blockDim.x) {
+    int t = idx >> LOGM, i = idx & (M - 1);
+    sm[t * P + fft_phys(i)] = in[(size_t)t * M + i];
+  }
+  __syncthreads();
+  block_fft<LOGM, +1>(sm, a.nb, P, a.tw);
+  float2* out = a.out + ((size_t)pl * M + r0) * a.n;
+  for (int idx = threadIdx.x; idx < a.nb * a.n; idx += blockDim.x) {
+    int t = idx / a.n, ix = idx - t * a.n, x = ix - a.n / 2;
+    float2 v = sm[t * P + fft_phys(fft_pos<LOGM>(x & (M - 1)))];
+    if (x & 1) { v.x = -v.x; v.y = -v.y; }
+    out[(size_t)t * a.n + ix] = v;
+  }
+}
+
+// S3: inverse FFT along xi2 (columns), cropped:  A[p][ix2][ix1] = (-1)^x2 sum_i2 T[pl][i2][ix1] e^{+2 pi i x2 i2/M}
+template <int LOGM>
+__global__ void __launch_bounds__(256) k_ifft_x2(IfftArgs a) {
+  constexpr int M = 1 << LOGM, P = fft_pitch(M);
+  extern __shared__ float2 sm[];
+  const int pl = blockIdx.y, c0 = blockIdx.x * a.nb;
+  const float2* in = a.in + (size_t)pl * M * a.n + c0;
+  for (int idx = threadIdx.x; idx < a.nb << LOGM; idx += blockDim.x) {
+    int i = idx / a.nb, c = idx - i * a.nb;
+    sm[c * P + fft_phys(i)] = in[(size_t)i * a.n + c];
+  }
+  __syncthreads();
+  block_fft<LOGM, +1>(sm, a.nb, P, a.tw);
+  float2* out = a.out + (size_t)pl * a.n * a.n + c0;
+  for (int idx = threadIdx.x; idx < a.nb * a.n; idx += blockDim.x) {
+    int ix = idx / a.nb, c = idx - ix * a.nb, x = ix - a.n / 2;
+    float2 v = sm[c * P + fft_phys(fft_pos<LOGM>(x & (M - 1)))];
+    if (x & 1) { v.x = -v.x; v.y = -v.y; }
+    out[(size_t)ix * a.n + c] = v;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// x3 stage, one block per (x2, group of cb x1): xi3 = k_v cos(phi)/h depends on k_v only (Eq. 6), so the planes
+// A[p] are samples of a 1-D unequally spaced spectrum along x3 for every (x1, x2):
+//   Gz[m3] = sum_p A[p] kap(t3(p) - m3),  t3 = M3 k_v cos(phi)/h;   vol[x3] = Re sum_m3 Gz[m3] e^{2 pi i x3 m3/M3}
+//   divided by kaphat(x1/M) kaphat(x2/M) kaphat(x3/M3)  (PAPER.md:136 step 1, reversed per PAPER.md:140).
+// ---------------------------------------------------------------------------------------------------------------
+struct ZArgs {
+  const float2* A;       // [h/2+1][n][n]
+  float* vol;            // output buffer; element (ix3, ix2, ix1) at vol[ix3*zstride + (ix2 - vol_x2_0)*n + ix1]
+  size_t zstride;
+  const float2* tw;      // length M3
+  const float* wz;       // [h/2+1][W] tap weights of plane p
+  const int* bz;         // [h/2+1] first tap m3 of plane p
+  const int2* prange;    // [M3] planes [lo, hi] (p < h/2 only) with a tap on stored index i (= m3 mod M3); lo > hi: none
+  const float* dx;       // [n]  1/kaphat(x/M)
+  const float* dz;       // [nz] 1/kaphat(x3/M3)
+  int n, nz, np, cb, W;
+  int x2_0;              // first x2 row of this launch
+  int vol_x2_0;          // x2 index held by row 0 of the output buffer
+};
+
+template <int LOGM3>
+__global__ void __launch_bounds__(256) k_zstage(ZArgs a) {
+  constexpr int M3 = 1 << LOGM3, P = fft_pitch(M3);
+  extern __shared__ float2 sm[];
+  float2* Ain = sm;                       // [np][cb]
+  float2* Gz = sm + (size_t)a.np * a.cb;  // [cb][P]
+  const int ix2 = a.x2_0 + blockIdx.y, c0 = blockIdx.x * a.cb;
+  const size_t nn = (size_t)a.n * a.n;
+  const float2* Ab = a.A + (size_t)ix2 * a.n + c0;
+  for (int idx = threadIdx.x; idx < a.np * a.cb; idx += blockDim.x) {
+    int p = idx / a.cb, c = idx - p * a.cb;
+    Ain[idx] = Ab[(size_t)p * nn + c];
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < a.cb << LOGM3; idx += blockDim.x) {
+    int i = idx / a.cb, c = idx - i * a.cb;
+    int2 pr = a.prange[i];
+    float2 acc = make_float2(0.f, 0.f);
+    for (int p = pr.x; p <= pr.y; ++p) {
+      int j = (i - a.bz[p]) & (M3 - 1);
+      if (j < a.W) {
+        float wv = a.wz[p * a.W + j];
+        float2 v = Ain[p * a.cb + c];
+        acc.x = fmaf(v.x, wv, acc.x);
+        acc.y = fmaf(v.y, wv, acc.y);
+      }
+    }
+    Gz[c * P + fft_phys(i)] = acc;
+  }
+  __syncthreads();
+  {  // the k_v = -h/2 plane (p = np-1) is out of order: scatter its W taps (one thread per (tap, column))
+    int p = a.np - 1;
+    for (int idx = threadIdx.x; idx < a.W * a.cb; idx += blockDim.x) {
+      int j = idx / a.cb, c = idx - j * a.cb;
+      int m = a.bz[p] + j, i = m & (M3 - 1);
+      float wv = a.wz[p * a.W + j];
+      float2 v = Ain[p * a.cb + c];
+      float2* g = &Gz[c * P + fft_phys(i)];
+      g->x = fmaf(v.x, wv, g->x);
+      g->y = fmaf(v.y, wv, g->y);
+    }
+  }
+  __syncthreads();
+  block_fft<LOGM3, +1>(Gz, a.cb, P, a.tw);
+  const float dx2 = a.dx[ix2];
+  float* vb = a.vol + (size_t)(ix2 - a.vol_x2_0) * a.n + c0;
+  for (int idx = threadIdx.x; idx < a.nz * a.cb; idx += blockDim.x) {
+    int ix3 = idx / a.cb, c = idx - ix3 * a.cb, x3 = ix3 - a.nz / 2;
+    float v = Gz[c * P + fft_phys(fft_pos<LOGM3>(x3 & (M3 - 1)))].x;
+    vb[(size_t)ix3 * a.zstride + c] = v * a.dz[ix3] * dx2 * a.dx[c0 + c];
+  }
+}
+
+}  // namespace lam
