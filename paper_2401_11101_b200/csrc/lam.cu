@@ -1,0 +1,613 @@
+// lam.cu — host side of liblam.so: the C ABI of include/lam.h, the plan (tables, work lists, workspace) and the
+// launch schedule of the sm_100a kernels in lam_kernels.cuh.  No CPU fallback: every compute entry point needs a
+// CUDA device and returns LAM_ECUDA without one.
+//
+// Schedule of lam_backproject (Eq. 7 evaluated in the order of Eq. 9):
+//   for every chunk of projections:   k_rows  (S0 + row FFT + filter)  ->  k_cols (column FFT, fold onto k_v >= 0 planes)
+//   for every batch of k_v planes:    k_spread (gridding in xi1, xi2)  ->  k_ifft_x1  ->  k_ifft_x2  (cropped n x n planes)
+//   once:                             k_zstage (gridding in xi3 + inverse FFT + crop + real part + deapodisation)
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/lam.h"
+#include "lam_kernels.cuh"
+
+using namespace lam;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct StageEvent {
+  int stage;
+  cudaEvent_t a, b;
+};
+
+}  // namespace
+
+struct lam_plan {
+  // problem
+  int n = 0, nz = 0, h = 0, w = 0, ntheta = 0;
+  double phi = 0;
+  lam_params prm{};
+  std::vector<double> theta;
+  // derived
+  int M = 0, M3 = 0, W = 0, NP = 0, WR = 0, WQ = 0;
+  int logw = 0, logh = 0, logM = 0, logM3 = 0;
+  int PB = 1, TC = 1;  // plane batch, theta chunk
+  int rows_nb = 1, cols_cb = 1, x1_nb = 1, x2_nb = 1, z_cb = 1;
+  GridKernel gk;
+  KerPoly kp{};
+  SpreadGeom geom{};
+  // device tables
+  double2* d_cs = nullptr;
+  float2 *d_Pu = nullptr, *d_Pv = nullptr, *d_PuNone = nullptr;
+  float2 *d_tw_w = nullptr, *d_tw_h = nullptr, *d_tw_M = nullptr, *d_tw_M3 = nullptr;
+  float *d_wz = nullptr, *d_dx = nullptr, *d_dz = nullptr, *d_dark = nullptr, *d_flat = nullptr;
+  int* d_bz = nullptr;
+  int2* d_prange = nullptr;
+  uint2* d_jobs = nullptr;
+  std::vector<long long> job_off;  // [NP+1] first job of each plane
+  // workspace
+  float2 *d_R = nullptr, *d_S = nullptr, *d_G = nullptr, *d_T = nullptr, *d_A = nullptr;
+  size_t device_bytes = 0, pinned_bytes = 0;
+  bool have_darkflat = false;
+  // bookkeeping
+  std::string err;
+  int device = 0;
+  bool profiling = false;
+  std::vector<StageEvent> events;
+  size_t events_used = 0;
+  long long launches = 0;
+  float last_ms[6] = {0, 0, 0, 0, 0, 0};
+  bool stage_valid = false;
+};
+
+namespace {
+
+lam_status fail(lam_plan* p, lam_status st, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (p) p->err = buf;
+  else g_create_error = buf;
+  return st;
+}
+
+#define CU(p, call)                                                                                              \
+  do {                                                                                                           \
+    cudaError_t e_ = (call);                                                                                     \
+    if (e_ != cudaSuccess)                                                                                       \
+      return fail(p, e_ == cudaErrorMemoryAllocation ? LAM_ENOMEM_DEVICE : LAM_ECUDA, "%s: %s (%s:%d)", #call,   \
+                  cudaGetErrorString(e_), __FILE__, __LINE__);                                                   \
+  } while (0)
+
+int ilog2(int v) {
+  int l = 0;
+  while ((1 << l) < v) ++l;
+  return l;
+}
+bool pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+
+template <class T>
+lam_status dalloc(lam_plan* p, T** ptr, size_t count) {
+  size_t bytes = std::max<size_t>(count, 1) * sizeof(T);
+  cudaError_t e = cudaMalloc((void**)ptr, bytes);
+  if (e != cudaSuccess) {
+    *ptr = nullptr;
+    cudaGetLastError();
+    return fail(p, LAM_ENOMEM_DEVICE, "cudaMalloc of %zu bytes failed: %s", bytes, cudaGetErrorString(e));
+  }
+  p->device_bytes += bytes;
+  return LAM_OK;
+}
+
+template <class T>
+lam_status upload(lam_plan* p, T** ptr, const std::vector<T>& v) {
+  lam_status st = dalloc(p, ptr, v.size());
+  if (st != LAM_OK) return st;
+  CU(p, cudaMemcpy(*ptr, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice));
+  return LAM_OK;
+}
+
+std::vector<float2> twiddles(int N) {
+  std::vector<float2> t(N);
+  for (int k = 0; k < N; ++k) {
+    double a = -2.0 * kPi * k / N;
+    t[k] = make_float2((float)std::cos(a), (float)std::sin(a));
+  }
+  return t;
+}
+
+// ---- templated launch tables (FFT lengths 2^5 .. 2^13) ------------------------------------------------------------
+constexpr int kLogMin = 5, kLogMax = 13;
+
+template <int L>
+struct Launch {
+  static void rows(bool raw, dim3 g, size_t sm, cudaStream_t s, const RowsArgs& a) {
+    if (raw) {
+      cudaFuncSetAttribute(k_rows<L, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+      k_rows<L, true><<<g, 256, sm, s>>>(a);
+    } else {
+      cudaFuncSetAttribute(k_rows<L, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+      k_rows<L, false><<<g, 256, sm, s>>>(a);
+    }
+  }
+  static void cols(dim3 g, size_t sm, cudaStream_t s, const ColsArgs& a) {
+    cudaFuncSetAttribute(k_cols<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_cols<L><<<g, 256, sm, s>>>(a);
+  }
+  static void x1(dim3 g, size_t sm, cudaStream_t s, const IfftArgs& a) {
+    cudaFuncSetAttribute(k_ifft_x1<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_ifft_x1<L><<<g, 256, sm, s>>>(a);
+  }
+  static void x2(dim3 g, size_t sm, cudaStream_t s, const IfftArgs& a) {
+    cudaFuncSetAttribute(k_ifft_x2<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_ifft_x2<L><<<g, 256, sm, s>>>(a);
+  }
+  static void z(dim3 g, size_t sm, cudaStream_t s, const ZArgs& a) {
+    cudaFuncSetAttribute(k_zstage<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_zstage<L><<<g, 256, sm, s>>>(a);
+  }
+};
+
+template <int L, class F>
+void dispatch_log_impl(int lg, F&& f) {
+  if constexpr (L <= kLogMax) {
+    if (lg == L) f(Launch<L>{});
+    else dispatch_log_impl<L + 1>(lg, f);
+  }
+}
+#define DISPATCH_LOG(lg, call) dispatch_log_impl<kLogMin>(lg, [&](auto L_) { decltype(L_)::call; })
+
+template <class F>
+void dispatch_W(int W, F&& f) {
+  if (W == 4) f(std::integral_constant<int, 4>{});
+  else if (W == 6) f(std::integral_constant<int, 6>{});
+  else f(std::integral_constant<int, 8>{});
+}
+
+// ---- profiling events ----------------------------------------------------------------------------------------------
+struct StageScope {
+  lam_plan* p;
+  cudaStream_t s;
+  StageEvent* ev = nullptr;
+  StageScope(lam_plan* p_, int stage, cudaStream_t s_) : p(p_), s(s_) {
+    if (!p->profiling) return;
+    if (p->events_used == p->events.size()) {
+      StageEvent e{stage, nullptr, nullptr};
+      cudaEventCreate(&e.a);
+      cudaEventCreate(&e.b);
+      p->events.push_back(e);
+    }
+    ev = &p->events[p->events_used++];
+    ev->stage = stage;
+    cudaEventRecord(ev->a, s);
+  }
+  ~StageScope() {
+    if (ev) cudaEventRecord(ev->b, s);
+  }
+};
+
+void free_all(lam_plan* p) {
+  void* ptrs[] = {p->d_cs,    p->d_Pu,  p->d_Pv,  p->d_PuNone, p->d_tw_w, p->d_tw_h,   p->d_tw_M, p->d_tw_M3,
+                  p->d_wz,    p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_bz,     p->d_prange, p->d_jobs,
+                  p->d_R,     p->d_S,   p->d_G,   p->d_T,      p->d_A};
+  for (void* q : ptrs)
+    if (q) cudaFree(q);
+  for (auto& e : p->events) {
+    cudaEventDestroy(e.a);
+    cudaEventDestroy(e.b);
+  }
+}
+
+// ---- work lists of the (xi1, xi2) gridding: geometry only, built once ---------------------------------------------
+lam_status build_jobs(lam_plan* p) {
+  const int ntiles = p->geom.nt * p->geom.nt;
+  const int chunk = std::max(1, std::min(p->NP, (1 << 23) / ntiles));
+  unsigned *d_count = nullptr, *d_off = nullptr;
+  size_t scratch = (size_t)chunk * ntiles;
+  if (cudaMalloc(&d_count, scratch * 4) != cudaSuccess || cudaMalloc(&d_off, scratch * 4) != cudaSuccess) {
+    cudaGetLastError();
+    if (d_count) cudaFree(d_count);
+    return fail(p, LAM_ENOMEM_DEVICE, "work-list scratch of %zu bytes does not fit", scratch * 8);
+  }
+  std::vector<unsigned> counts((size_t)p->NP * ntiles);
+  lam_status st = LAM_OK;
+  auto launch = [&](int p0, int np, bool fill, uint2* jobs) {
+    JobsArgs a{p->geom, p0, np, d_count, d_off, jobs};
+    long long total = (long long)np * ntiles;
+    unsigned blocks = (unsigned)((total + 127) / 128);
+    dispatch_W(p->W, [&](auto Wc) {
+      constexpr int W = decltype(Wc)::value;
+      if (fill) k_jobs<W, true><<<blocks, 128>>>(a);
+      else k_jobs<W, false><<<blocks, 128>>>(a);
+    });
+  };
+  for (int p0 = 0; p0 < p->NP && st == LAM_OK; p0 += chunk) {
+    int np = std::min(chunk, p->NP - p0);
+    launch(p0, np, false, nullptr);
+    cudaError_t e = cudaMemcpy(counts.data() + (size_t)p0 * ntiles, d_count, (size_t)np * ntiles * 4, cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) st = fail(p, LAM_ECUDA, "work-list count pass: %s", cudaGetErrorString(e));
+  }
+  if (st == LAM_OK) {
+    p->job_off.assign(p->NP + 1, 0);
+    long long tot = 0;
+    for (int pl = 0; pl < p->NP; ++pl) {
+      p->job_off[pl] = tot;
+      for (int t = 0; t < ntiles; ++t) tot += counts[(size_t)pl * ntiles + t];
+    }
+    p->job_off[p->NP] = tot;
+    st = dalloc(p, &p->d_jobs, (size_t)tot);
+  }
+  std::vector<unsigned> offs(scratch);
+  for (int p0 = 0; p0 < p->NP && st == LAM_OK; p0 += chunk) {
+    int np = std::min(chunk, p->NP - p0);
+    unsigned run = 0;
+    for (size_t i = 0; i < (size_t)np * ntiles; ++i) {
+      offs[i] = run;
+      run += counts[(size_t)p0 * ntiles + i];
+    }
+    cudaMemcpy(d_off, offs.data(), (size_t)np * ntiles * 4, cudaMemcpyHostToDevice);
+    cudaMemcpy(d_count, counts.data() + (size_t)p0 * ntiles, (size_t)np * ntiles * 4, cudaMemcpyHostToDevice);
+    launch(p0, np, true, p->d_jobs + p->job_off[p0]);
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) st = fail(p, LAM_ECUDA, "work-list fill pass: %s", cudaGetErrorString(e));
+  }
+  cudaFree(d_count);
+  cudaFree(d_off);
+  return st;
+}
+
+lam_status make_tables(lam_plan* p) {
+  lam_status st;
+  const int n = p->n, nz = p->nz, h = p->h, w = p->w, M = p->M, M3 = p->M3, W = p->W, NP = p->NP;
+  const double sigma = p->prm.oversample;
+  // angles
+  std::vector<double2> cs(p->ntheta);
+  for (int t = 0; t < p->ntheta; ++t) cs[t] = make_double2(std::cos(p->theta[t]), std::sin(p->theta[t]));
+  if ((st = upload(p, &p->d_cs, cs)) != LAM_OK) return st;
+  // filter x centring phase x 1/(wh) along k_u; centring phase along k_v
+  const double cu = std::isnan(p->prm.center_u) ? 0.5 * w : (double)p->prm.center_u;
+  const double cv = std::isnan(p->prm.center_v) ? 0.5 * h : (double)p->prm.center_v;
+  for (int pass = 0; pass < 2; ++pass) {
+    std::vector<double> H;
+    filter_response(pass == 0 ? p->prm.filter : 0, w, p->phi, p->ntheta, H);
+    std::vector<float2> Pu(w / 2 + 1);
+    for (int k = 0; k <= w / 2; ++k) {
+      double a = 2.0 * kPi * std::fmod((double)k * cu, (double)w) / w, s = H[k] / ((double)w * h);
+      Pu[k] = make_float2((float)(s * std::cos(a)), (float)(s * std::sin(a)));
+    }
+    if ((st = upload(p, pass == 0 ? &p->d_Pu : &p->d_PuNone, Pu)) != LAM_OK) return st;
+  }
+  std::vector<float2> Pv(NP);
+  for (int q = 0; q < NP; ++q) {
+    int kv = q == h / 2 ? -h / 2 : q;
+    double a = 2.0 * kPi * std::fmod((double)kv * cv, (double)h) / h;
+    Pv[q] = make_float2((float)std::cos(a), (float)std::sin(a));
+  }
+  if ((st = upload(p, &p->d_Pv, Pv)) != LAM_OK) return st;
+  if ((st = upload(p, &p->d_tw_w, twiddles(w))) != LAM_OK) return st;
+  if ((st = upload(p, &p->d_tw_h, twiddles(h))) != LAM_OK) return st;
+  if ((st = upload(p, &p->d_tw_M, twiddles(M))) != LAM_OK) return st;
+  if ((st = upload(p, &p->d_tw_M3, twiddles(M3))) != LAM_OK) return st;
+  // gridding kernel: polynomial pieces for (xi1, xi2); explicit weights for xi3 (they depend on k_v only)
+  p->gk.init(p->prm.kernel, W, sigma, p->prm.shape);
+  kernel_poly(p->gk, &p->kp.E[0][0], &p->kp.O[0][0]);
+  std::vector<float> wz((size_t)NP * W);
+  std::vector<int> bz(NP);
+  std::vector<int2> prange(M3, make_int2(1, 0));
+  const double cphi = std::cos(p->phi);
+  for (int q = 0; q < NP; ++q) {
+    int kv = q == h / 2 ? -h / 2 : q;
+    double t3 = (double)M3 * kv * cphi / h;
+    int b = (int)std::ceil(t3 - 0.5 * W);
+    bz[q] = b;
+    for (int j = 0; j < W; ++j) wz[(size_t)q * W + j] = (float)p->gk.kap(t3 - (b + j));
+    if (q < h / 2)
+      for (int j = 0; j < W; ++j) {
+        int i = ((b + j) % M3 + M3) % M3;
+        if (prange[i].x > prange[i].y) prange[i] = make_int2(q, q);
+        else { prange[i].x = std::min(prange[i].x, q); prange[i].y = std::max(prange[i].y, q); }
+      }
+  }
+  if ((st = upload(p, &p->d_wz, wz)) != LAM_OK) return st;
+  if ((st = upload(p, &p->d_bz, bz)) != LAM_OK) return st;
+  if ((st = upload(p, &p->d_prange, prange)) != LAM_OK) return st;
+  std::vector<float> dx(n), dz(nz);
+  for (int i = 0; i < n; ++i) dx[i] = (float)(1.0 / p->gk.kaphat((double)(i - n / 2) / M));
+  for (int i = 0; i < nz; ++i) dz[i] = (float)(1.0 / p->gk.kaphat((double)(i - nz / 2) / M3));
+  if ((st = upload(p, &p->d_dx, dx)) != LAM_OK) return st;
+  if ((st = upload(p, &p->d_dz, dz)) != LAM_OK) return st;
+  // geometry of the (xi1, xi2) gridding
+  SpreadGeom& g = p->geom;
+  g.cs = p->d_cs;
+  g.rho_unit = (double)M * std::sin(p->phi) / h;
+  g.a1 = (float)M / (float)w;
+  g.M = M;
+  g.nt = M / kTile;
+  g.ntheta = p->ntheta;
+  g.w = w;
+  g.hh = h / 2;
+  g.kstride = std::max(1, (int)std::ceil(1.0002 * std::sqrt(2.0) * w / M));
+  return LAM_OK;
+}
+
+size_t zstage_smem(const lam_plan* p, int cb) { return ((size_t)p->NP * cb + (size_t)cb * fft_pitch(p->M3)) * sizeof(float2); }
+
+}  // namespace
+
+// ====================================================================================================================
+extern "C" {
+
+const char* lam_version(void) { return "lam-b200 0.1 (sm_100a)"; }
+
+void lam_default_params(lam_params* p) {
+  if (!p) return;
+  memset(p, 0, sizeof *p);
+  p->nz = 0;
+  p->kernel = LAM_KERNEL_KB;
+  p->width = 6;
+  p->oversample = 2.0f;
+  p->shape = 0.f;
+  p->filter = LAM_FILTER_RAMP;
+  p->input = LAM_INPUT_F32;
+  p->center_u = NAN;
+  p->center_v = NAN;
+  p->t_min = 1e-6f;
+  p->device_bytes = 0;
+  p->plane_batch = 0;
+  p->theta_chunk = 0;
+}
+
+const char* lam_last_error(const lam_plan* plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
+
+void lam_destroy(lam_plan* plan) {
+  if (!plan) return;
+  cudaSetDevice(plan->device);
+  free_all(plan);
+  delete plan;
+}
+
+lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const float* theta_rad, const lam_params* prm,
+                      lam_plan** out) {
+  if (!out) return fail(nullptr, LAM_EINVAL, "out is NULL");
+  *out = nullptr;
+  lam_params P;
+  if (prm) P = *prm;
+  else lam_default_params(&P);
+  if (P.nz == 0) P.nz = n;
+  if (P.width == 0) P.width = 6;
+  if (P.oversample == 0.f) P.oversample = 2.0f;
+  if (P.t_min == 0.f) P.t_min = 1e-6f;
+  if (n < 2 || h < 2 || w < 2 || P.nz < 2 || n_theta < 1 || !theta_rad)
+    return fail(nullptr, LAM_EINVAL, "n, nz, h, w must be >= 2, n_theta >= 1, theta not NULL");
+  if ((n | h | w | P.nz) & 1) return fail(nullptr, LAM_EINVAL, "n, nz, h, w must be even");
+  if (!(phi_rad >= 0.f) || !(phi_rad < 1.5707963f)) return fail(nullptr, LAM_EINVAL, "phi must be in [0, pi/2)");
+  if (P.kernel != LAM_KERNEL_KB && P.kernel != LAM_KERNEL_GAUSS) return fail(nullptr, LAM_EINVAL, "unknown kernel");
+  if (P.filter < 0 || P.filter > 2) return fail(nullptr, LAM_EINVAL, "unknown filter");
+  if (P.input != LAM_INPUT_F32 && P.input != LAM_INPUT_U16_RAW) return fail(nullptr, LAM_EINVAL, "unknown input type");
+  if (P.width != 4 && P.width != 6 && P.width != 8) return fail(nullptr, LAM_EUNSUPPORTED, "width must be 4, 6 or 8");
+  if (!(P.oversample >= 1.25f) || !(P.oversample <= 4.f)) return fail(nullptr, LAM_EINVAL, "oversample must be in [1.25, 4]");
+  if (!(P.shape >= 0.f)) return fail(nullptr, LAM_EINVAL, "shape must be >= 0");
+  double Md = (double)P.oversample * n, M3d = (double)P.oversample * P.nz;
+  int M = (int)std::lround(Md), M3 = (int)std::lround(M3d);
+  if (std::fabs(Md - M) > 1e-6 || std::fabs(M3d - M3) > 1e-6 || !pow2(M) || !pow2(M3) || !pow2(w) || !pow2(h))
+    return fail(nullptr, LAM_EUNSUPPORTED, "w, h, sigma*n and sigma*nz must be powers of two (got %d, %d, %g, %g)", w, h, Md, M3d);
+  const int lo = 1 << kLogMin, hi = 1 << kLogMax;
+  if (w < lo || w > hi || h < lo || h > hi || M < 64 || M > hi || M3 < lo || M3 > hi)
+    return fail(nullptr, LAM_EUNSUPPORTED, "w, h, sigma*nz must be in [32, 8192] and sigma*n in [64, 8192]");
+  if (h / 2 + 1 > 0x1fff || M / kTile > 0x1ff || n_theta > 0x3fff)
+    return fail(nullptr, LAM_EUNSUPPORTED, "h <= 16382, sigma*n <= 16352 and n_theta <= 16383 in this build");
+  if (M3 < 2 * P.width || M < 2 * P.width) return fail(nullptr, LAM_EINVAL, "grid smaller than the kernel footprint");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(nullptr, LAM_ECUDA, "no CUDA device (this library has no CPU path)");
+  }
+  lam_plan* p = new (std::nothrow) lam_plan;
+  if (!p) return fail(nullptr, LAM_ENOMEM_HOST, "out of host memory");
+  cudaGetDevice(&p->device);
+  p->n = n; p->nz = P.nz; p->h = h; p->w = w; p->ntheta = n_theta; p->phi = phi_rad; p->prm = P;
+  p->theta.assign(theta_rad, theta_rad + n_theta);
+  p->M = M; p->M3 = M3; p->W = P.width; p->NP = h / 2 + 1;
+  p->WR = (w / 2 + 1 + 7) & ~7;
+  p->WQ = (w + 1 + 7) & ~7;
+  p->logw = ilog2(w); p->logh = ilog2(h); p->logM = ilog2(M); p->logM3 = ilog2(M3);
+
+  auto bail = [&](lam_status st) {
+    g_create_error = p->err;
+    free_all(p);
+    delete p;
+    return st;
+  };
+  lam_status st = make_tables(p);
+  if (st != LAM_OK) return bail(st);
+
+  // block shapes
+  p->rows_nb = std::min(h / 2, std::max(1, 4096 / w));
+  p->cols_cb = std::max(2, std::min(32, 8192 / h));
+  p->x1_nb = std::max(1, std::min(M, 4096 / M));
+  p->x2_nb = std::min(n, std::max(2, std::min(32, 16384 / M)));
+  {
+    int cb = 32;
+    while (cb > 1 && (zstage_smem(p, cb) > 110 * 1024 || n % cb)) cb >>= 1;
+    if (zstage_smem(p, cb) > 220 * 1024) return bail(fail(p, LAM_EUNSUPPORTED, "x3 stage does not fit shared memory (h = %d, sigma*nz = %d)", h, M3));
+    p->z_cb = cb;
+  }
+  // workspace: batch sizes from the budget
+  size_t freeb = 0, totalb = 0;
+  if (cudaMemGetInfo(&freeb, &totalb) != cudaSuccess) return bail(fail(p, LAM_ECUDA, "cudaMemGetInfo failed"));
+  size_t budget = P.device_bytes ? P.device_bytes : (size_t)(0.9 * (double)freeb);
+  const size_t gplane = (size_t)M * M * 8, tplane = (size_t)M * n * 8;
+  p->PB = P.plane_batch > 0 ? P.plane_batch : (int)std::max<size_t>(1, std::min<size_t>(p->NP, (96u << 20) / (gplane + tplane)));
+  p->PB = std::min(p->PB, p->NP);
+  const size_t rproj = (size_t)h * p->WR * 8;
+  p->TC = P.theta_chunk > 0 ? P.theta_chunk : (int)std::max<size_t>(1, std::min<size_t>(n_theta, (32u << 20) / rproj));
+  p->TC = std::min(p->TC, n_theta);
+  const size_t need = (size_t)p->TC * rproj + (size_t)p->NP * n_theta * p->WQ * 8 + (size_t)p->PB * (gplane + tplane) +
+                      (size_t)p->NP * n * n * 8 + p->device_bytes;
+  if (need > budget)
+    return bail(fail(p, LAM_ENOMEM_DEVICE, "in-core workspace of %.2f GB exceeds the budget of %.2f GB", need / 1e9, budget / 1e9));
+  if ((st = dalloc(p, &p->d_R, (size_t)p->TC * h * p->WR)) != LAM_OK) return bail(st);
+  if ((st = dalloc(p, &p->d_S, (size_t)p->NP * n_theta * p->WQ)) != LAM_OK) return bail(st);
+  if ((st = dalloc(p, &p->d_G, (size_t)p->PB * M * M)) != LAM_OK) return bail(st);
+  if ((st = dalloc(p, &p->d_T, (size_t)p->PB * M * n)) != LAM_OK) return bail(st);
+  if ((st = dalloc(p, &p->d_A, (size_t)p->NP * n * n)) != LAM_OK) return bail(st);
+  if ((st = build_jobs(p)) != LAM_OK) return bail(st);
+  // the q = w slot and the row padding of S are read by k_spread: keep them defined
+  if (cudaMemset(p->d_S, 0, (size_t)p->NP * n_theta * p->WQ * 8) != cudaSuccess) return bail(fail(p, LAM_ECUDA, "memset failed"));
+  if (cudaDeviceSynchronize() != cudaSuccess) return bail(fail(p, LAM_ECUDA, "plan setup failed: %s", cudaGetErrorString(cudaGetLastError())));
+  *out = p;
+  return LAM_OK;
+}
+
+lam_status lam_set_darkflat(lam_plan* p, const float* dark, const float* flat) {
+  if (!p) return LAM_EINVAL;
+  if (!dark || !flat) return fail(p, LAM_EINVAL, "dark / flat is NULL");
+  cudaSetDevice(p->device);
+  size_t cnt = (size_t)p->h * p->w;
+  lam_status st;
+  if (!p->d_dark && (st = dalloc(p, &p->d_dark, cnt)) != LAM_OK) return st;
+  if (!p->d_flat && (st = dalloc(p, &p->d_flat, cnt)) != LAM_OK) return st;
+  CU(p, cudaMemcpy(p->d_dark, dark, cnt * 4, cudaMemcpyDefault));
+  CU(p, cudaMemcpy(p->d_flat, flat, cnt * 4, cudaMemcpyDefault));
+  p->have_darkflat = true;
+  return LAM_OK;
+}
+
+lam_status lam_set_profiling(lam_plan* p, int on) {
+  if (!p) return LAM_EINVAL;
+  p->profiling = on != 0;
+  return LAM_OK;
+}
+
+static bool is_device_ptr(const void* q) {
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, q) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+// S0 + S1 for projections [th0, th0 + nth) at device pointer `chunk` (the first projection of the chunk)
+static void launch_s1(lam_plan* p, const void* chunk, int th0, int nth, cudaStream_t s) {
+  const bool raw = p->prm.input == LAM_INPUT_U16_RAW;
+  RowsArgs ra{chunk, p->d_dark, p->d_flat, p->prm.t_min, p->d_R, p->d_Pu, p->d_tw_w, p->h, p->WR, p->rows_nb};
+  dim3 gr(p->h / 2 / p->rows_nb, nth);
+  size_t smr = (size_t)p->rows_nb * fft_pitch(p->w) * sizeof(float2);
+  DISPATCH_LOG(p->logw, rows(raw, gr, smr, s, ra));
+  ColsArgs ca{p->d_R, p->d_S, p->d_Pv, p->d_tw_h, p->w, p->WR, p->WQ, p->ntheta, th0, p->cols_cb};
+  dim3 gc((p->w / 2 + 1 + p->cols_cb - 1) / p->cols_cb, nth);
+  size_t smc = (size_t)p->cols_cb * fft_pitch(p->h) * sizeof(float2);
+  DISPATCH_LOG(p->logh, cols(gc, smc, s, ca));
+  p->launches += 2;
+}
+
+// S2 + S3 (x1, x2) for planes [p0, p0 + np)
+static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
+  SpreadArgs sa{p->geom, p->kp, p->d_jobs + p->job_off[p0], p->job_off[p0 + np] - p->job_off[p0], p->d_S, p->WQ, p->d_G, p0};
+  {
+    StageScope sc(p, 1, s);
+    unsigned blocks = (unsigned)((sa.njobs + kSpreadWarps - 1) / kSpreadWarps);
+    k_zero_tiles<<<blocks, kSpreadWarps * 32, 0, s>>>(sa);
+    size_t sm = (size_t)kSpreadWarps * kTile * kTilePitch * sizeof(float2);
+    dispatch_W(p->W, [&](auto Wc) {
+      constexpr int W = decltype(Wc)::value;
+      cudaFuncSetAttribute(k_spread<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+      k_spread<W><<<blocks, kSpreadWarps * 32, sm, s>>>(sa);
+    });
+  }
+  {
+    StageScope sc(p, 2, s);
+    IfftArgs a1{p->d_G, p->d_T, p->d_tw_M, p->n, p->x1_nb};
+    DISPATCH_LOG(p->logM, x1(dim3(p->M / p->x1_nb, np), (size_t)p->x1_nb * fft_pitch(p->M) * sizeof(float2), s, a1));
+    IfftArgs a2{p->d_T, p->d_A + (size_t)p0 * p->n * p->n, p->d_tw_M, p->n, p->x2_nb};
+    DISPATCH_LOG(p->logM, x2(dim3(p->n / p->x2_nb, np), (size_t)p->x2_nb * fft_pitch(p->M) * sizeof(float2), s, a2));
+  }
+  p->launches += 4;
+}
+
+static void launch_z(lam_plan* p, float* vol, cudaStream_t s) {
+  StageScope sc(p, 3, s);
+  ZArgs za{p->d_A, vol, (size_t)p->n * p->n, p->d_tw_M3, p->d_wz, p->d_bz, p->d_prange, p->d_dx, p->d_dz,
+           p->n, p->nz, p->NP, p->z_cb, p->W, 0, 0};
+  DISPATCH_LOG(p->logM3, z(dim3(p->n / p->z_cb, p->n), zstage_smem(p, p->z_cb), s, za));
+  p->launches += 1;
+}
+
+lam_status lam_backproject(lam_plan* p, const void* proj, float* vol, void* cuda_stream) {
+  if (!p) return LAM_EINVAL;
+  if (!proj || !vol) return fail(p, LAM_EINVAL, "proj / vol is NULL");
+  if (p->prm.input == LAM_INPUT_U16_RAW && !p->have_darkflat) return fail(p, LAM_EINVAL, "uint16 input needs lam_set_darkflat first");
+  cudaSetDevice(p->device);
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (!is_device_ptr(proj) || !is_device_ptr(vol))
+    return fail(p, LAM_EUNSUPPORTED, "host-pointer (out-of-core) path is not implemented in this build");
+  p->launches = 0;
+  p->events_used = 0;
+  p->stage_valid = false;
+  const size_t esz = p->prm.input == LAM_INPUT_U16_RAW ? 2 : 4;
+  {
+    StageScope total(p, 5, s);
+    {
+      StageScope sc(p, 0, s);
+      for (int th0 = 0; th0 < p->ntheta; th0 += p->TC) {
+        int nth = std::min(p->TC, p->ntheta - th0);
+        launch_s1(p, (const char*)proj + (size_t)th0 * p->h * p->w * esz, th0, nth, s);
+      }
+    }
+    for (int p0 = 0; p0 < p->NP; p0 += p->PB) launch_planes(p, p0, std::min(p->PB, p->NP - p0), s);
+    launch_z(p, vol, s);
+  }
+  CU(p, cudaGetLastError());
+  p->stage_valid = p->profiling;
+  return LAM_OK;
+}
+
+lam_status lam_forward(lam_plan* p, const float* vol, float* proj, void* cuda_stream) {
+  (void)vol; (void)proj; (void)cuda_stream;
+  if (!p) return LAM_EINVAL;
+  return fail(p, LAM_EUNSUPPORTED, "lam_forward is not implemented in this build");
+}
+
+lam_status lam_stage_ms(lam_plan* p, float ms[6]) {
+  if (!p || !ms) return LAM_EINVAL;
+  if (!p->stage_valid) return fail(p, LAM_EINVAL, "no profiled lam_backproject to report (lam_set_profiling(plan, 1) first)");
+  cudaSetDevice(p->device);
+  for (int i = 0; i < 6; ++i) ms[i] = 0.f;
+  for (size_t i = 0; i < p->events_used; ++i) {
+    StageEvent& e = p->events[i];
+    CU(p, cudaEventSynchronize(e.b));
+    float t = 0.f;
+    CU(p, cudaEventElapsedTime(&t, e.a, e.b));
+    ms[e.stage] += t;
+  }
+  return LAM_OK;
+}
+
+lam_status lam_plan_info(const lam_plan* p, long long info[8]) {
+  if (!p || !info) return LAM_EINVAL;
+  info[0] = (long long)p->device_bytes;
+  info[1] = p->NP;
+  info[2] = p->PB;
+  info[3] = p->job_off.empty() ? 0 : p->job_off.back();
+  info[4] = 0;
+  info[5] = p->TC;
+  info[6] = p->launches;
+  info[7] = (long long)p->pinned_bytes;
+  return LAM_OK;
+}
+
+}  // extern "C"
