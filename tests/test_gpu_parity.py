@@ -1,0 +1,164 @@
+"""GPU parity tests: the CUDA path (through the C ABI of include/lam.h) against the CPU fp64 oracle, element by
+element on the same seeded inputs.  Gates (BASELINE.json north_star): rel L2 <= 2e-4 against path A (exact NUDFT,
+Eq. 7) on configs[0]; <= 1e-3 against the oracle's double gridded path C / exact columns on larger cases.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import lam_oracle as O
+from paper_2401_11101_b200 import inputs, lam
+
+pytestmark = pytest.mark.gpu
+
+GATE_TINY = 2e-4   # north_star: configs[0] against the exact oracle
+GATE_LARGE = 1e-3  # north_star: larger configs against the oracle's gridded path / exact columns
+
+
+def rel(a, b):
+    a, b = np.asarray(a, dtype=np.float64), np.asarray(b, dtype=np.float64)
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def run_gpu(cfg, d, **kw):
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
+                    input="u16" if cfg.raw16 else "f32", **kw)
+    if cfg.raw16:
+        plan.set_darkflat(d["dark"].cuda(), d["flat"].cuda())
+    vol = plan.backproject(d["proj"].cuda())
+    torch.cuda.synchronize()
+    info = plan.info()
+    plan.close()
+    return vol.cpu().numpy(), info
+
+
+def geometry(cfg, d, **kw):
+    dark = d["dark"].numpy() if d["dark"] is not None else None
+    flat = d["flat"].numpy() if d["flat"] is not None else None
+    return O.Geometry(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, dark=dark, flat=flat, **kw)
+
+
+def test_version_and_native_library_loaded():
+    assert "sm_100a" in lam.lam_version()
+
+
+def test_config0_tiny_against_exact_nudft_full_volume():
+    cfg = inputs.config(0)
+    d = inputs.projections(cfg)
+    vol, info = run_gpu(cfg, d)
+    ref = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy())
+    assert vol.shape == ref.shape == (cfg.nz, cfg.n, cfg.n)
+    assert np.isfinite(vol).all()
+    assert rel(vol, ref) <= GATE_TINY
+    assert info["launches"] > 0
+
+
+@pytest.mark.parametrize("filt", ["none", "shepp-logan"])
+def test_config0_other_filters(filt):
+    cfg = inputs.config(0)
+    d = inputs.projections(cfg)
+    vol, _ = run_gpu(cfg, d, filter=filt)
+    ref = O.fbp_nudft(geometry(cfg, d, filter=filt), d["proj"].numpy())
+    assert rel(vol, ref) <= GATE_TINY
+
+
+def test_config0_gaussian_kernel_w8():
+    """The paper's psi is a Gaussian; at W = 8 it meets 1e-3 (reading Q5)."""
+    cfg = inputs.config(0)
+    d = inputs.projections(cfg)
+    vol, _ = run_gpu(cfg, d, kernel="gauss", width=8)
+    ref = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy())
+    assert rel(vol, ref) <= GATE_LARGE
+
+
+def test_config0_fractional_rotation_axis():
+    cfg = inputs.config(0)
+    d = inputs.projections(cfg)
+    cu, cv = cfg.w / 2 + 1.37, cfg.h / 2 - 0.61
+    vol, _ = run_gpu(cfg, d, center_u=cu, center_v=cv)
+    ref = O.fbp_nudft(geometry(cfg, d, cu=cu, cv=cv), d["proj"].numpy())
+    assert rel(vol, ref) <= GATE_TINY
+
+
+def test_small_batches_give_the_same_answer():
+    """plane_batch / theta_chunk only change the launch schedule (ragged last batch included)."""
+    cfg = inputs.config(0)
+    d = inputs.projections(cfg)
+    a, _ = run_gpu(cfg, d)
+    b, info = run_gpu(cfg, d, plane_batch=5, theta_chunk=7)
+    assert info["plane_batch"] == 5 and info["theta_chunk"] == 7
+    assert rel(b, a) <= 2e-6
+
+
+@pytest.mark.parametrize("idx,n", [(1, 128), (2, 128), (2, 256)])
+def test_scaled_configs_against_gridded_oracle(idx, n):
+    """Same recipes as configs[1], [2] shrunk so that the oracle's path C finishes in seconds; non-cubic slab
+    (nz = n/4, h != nz), phi = 20 / 30 degrees, noise, box layer; several gridding tiles and plane batches."""
+    cfg = inputs.scaled(idx, n)
+    d = inputs.projections(cfg)
+    vol, _ = run_gpu(cfg, d, plane_batch=24)
+    ref = O.fbp_gridded(geometry(cfg, d), d["proj"].numpy())
+    assert rel(vol, ref) <= GATE_LARGE
+    rng = np.random.default_rng(5)
+    cols = rng.integers(0, cfg.n, size=(16, 2)).astype(np.int32)
+    refA = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy(), cols=cols)     # [ncols][nz]
+    got = np.stack([vol[:, c[1], c[0]] for c in cols])
+    assert rel(got, refA) <= GATE_LARGE
+
+
+def test_raw_uint16_darkflat_path():
+    """configs[3] recipe (uint16 counts + dark/flat, -log fused) shrunk to n = 128."""
+    cfg = inputs.scaled(3, 128)
+    d = inputs.projections(cfg)
+    assert d["proj"].dtype == torch.uint16
+    vol, _ = run_gpu(cfg, d)
+    ref = O.fbp_gridded(geometry(cfg, d), d["proj"].numpy())
+    assert rel(vol, ref) <= GATE_LARGE
+
+
+def test_wide_detector_nonsquare():
+    """configs[4] recipe shrunk (w = 2 h, n = w): detector wider than tall."""
+    cfg = inputs.scaled(4, 128)
+    d = inputs.projections(cfg)
+    assert cfg.w == 2 * cfg.h
+    vol, _ = run_gpu(cfg, d)
+    ref = O.fbp_gridded(geometry(cfg, d), d["proj"].numpy())
+    assert rel(vol, ref) <= GATE_LARGE
+
+
+def test_phi_zero_is_slicewise_tomography():
+    """phi = 0 (the Radon transform): every detector row reconstructs its own slice."""
+    cfg = inputs.scaled(0, 64)
+    from dataclasses import replace
+    cfg = replace(cfg, phi_deg=0.0)
+    d = inputs.projections(cfg)
+    vol, _ = run_gpu(cfg, d)
+    ref = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy())
+    assert rel(vol, ref) <= GATE_TINY
+
+
+def test_repeat_calls_agree():
+    cfg = inputs.config(0)
+    d = inputs.projections(cfg)
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz)
+    p = d["proj"].cuda()
+    a = plan.backproject(p).clone()
+    b = plan.backproject(p)
+    torch.cuda.synchronize()
+    assert rel(b.cpu().numpy(), a.cpu().numpy()) <= 2e-6
+    plan.close()
+
+
+def test_errors_do_not_cross_the_boundary():
+    with pytest.raises(lam.LamError) as e:
+        lam.Plan(60, 64, 64, [0.0, 1.0], 0.3)          # sigma*n not a power of two
+    assert e.value.status == lam.LAM_EUNSUPPORTED
+    with pytest.raises(lam.LamError) as e:
+        lam.Plan(64, 64, 64, [0.0, 1.0], 2.0)          # phi out of range
+    assert e.value.status == lam.LAM_EINVAL
+    plan = lam.Plan(64, 64, 64, [0.0, 1.0], 0.3, input="u16")
+    with pytest.raises(lam.LamError):                   # dark/flat missing
+        plan.backproject(torch.zeros((2, 64, 64), dtype=torch.uint16, device="cuda"))
+    plan.close()
