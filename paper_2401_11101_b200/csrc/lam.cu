@@ -59,6 +59,13 @@ struct lam_plan {
   float2 *d_R = nullptr, *d_S = nullptr, *d_G = nullptr, *d_T = nullptr, *d_A = nullptr;
   size_t device_bytes = 0, pinned_bytes = 0;
   bool have_darkflat = false;
+  // host-pointer path (allocated on first use): device staging, copy streams, hand-over events
+  void* d_in[2] = {nullptr, nullptr};
+  float* d_out[2] = {nullptr, nullptr};
+  int ZR = 0;  // x2 rows per output slab
+  cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+  cudaEvent_t ev_in_ready[2] = {}, ev_in_free[2] = {}, ev_out_ready[2] = {}, ev_out_free[2] = {}, ev_fork = nullptr;
+  bool host_path_ready = false;
   // bookkeeping
   std::string err;
   int device = 0;
@@ -180,7 +187,7 @@ void dispatch_W(int W, F&& f) {
 struct StageScope {
   lam_plan* p;
   cudaStream_t s;
-  StageEvent* ev = nullptr;
+  long idx = -1;  // index, not pointer: nested scopes may grow the vector
   StageScope(lam_plan* p_, int stage, cudaStream_t s_) : p(p_), s(s_) {
     if (!p->profiling) return;
     if (p->events_used == p->events.size()) {
@@ -189,12 +196,12 @@ struct StageScope {
       cudaEventCreate(&e.b);
       p->events.push_back(e);
     }
-    ev = &p->events[p->events_used++];
-    ev->stage = stage;
-    cudaEventRecord(ev->a, s);
+    idx = (long)p->events_used++;
+    p->events[idx].stage = stage;
+    cudaEventRecord(p->events[idx].a, s);
   }
   ~StageScope() {
-    if (ev) cudaEventRecord(ev->b, s);
+    if (idx >= 0) cudaEventRecord(p->events[idx].b, s);
   }
 };
 
@@ -204,6 +211,17 @@ void free_all(lam_plan* p) {
                   p->d_R,     p->d_S,   p->d_G,   p->d_T,      p->d_A};
   for (void* q : ptrs)
     if (q) cudaFree(q);
+  for (int i = 0; i < 2; ++i) {
+    if (p->d_in[i]) cudaFree(p->d_in[i]);
+    if (p->d_out[i]) cudaFree(p->d_out[i]);
+    if (p->ev_in_ready[i]) cudaEventDestroy(p->ev_in_ready[i]);
+    if (p->ev_in_free[i]) cudaEventDestroy(p->ev_in_free[i]);
+    if (p->ev_out_ready[i]) cudaEventDestroy(p->ev_out_ready[i]);
+    if (p->ev_out_free[i]) cudaEventDestroy(p->ev_out_free[i]);
+  }
+  if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+  if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
+  if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
   for (auto& e : p->events) {
     cudaEventDestroy(e.a);
     cudaEventDestroy(e.b);
@@ -539,12 +557,36 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
   p->launches += 4;
 }
 
-static void launch_z(lam_plan* p, float* vol, cudaStream_t s) {
+// x3 stage for x2 rows [x2_0, x2_0 + rows); out holds x2 row `out_x2_0` in its first row, z-stride `zstride` floats
+static void launch_z(lam_plan* p, float* out, size_t zstride, int x2_0, int rows, int out_x2_0, cudaStream_t s) {
   StageScope sc(p, 3, s);
-  ZArgs za{p->d_A, vol, (size_t)p->n * p->n, p->d_tw_M3, p->d_wz, p->d_bz, p->d_prange, p->d_dx, p->d_dz,
-           p->n, p->nz, p->NP, p->z_cb, p->W, 0, 0};
-  DISPATCH_LOG(p->logM3, z(dim3(p->n / p->z_cb, p->n), zstage_smem(p, p->z_cb), s, za));
+  ZArgs za{p->d_A, out, zstride, p->d_tw_M3, p->d_wz, p->d_bz, p->d_prange, p->d_dx, p->d_dz,
+           p->n, p->nz, p->NP, p->z_cb, p->W, x2_0, out_x2_0};
+  DISPATCH_LOG(p->logM3, z(dim3(p->n / p->z_cb, rows), zstage_smem(p, p->z_cb), s, za));
   p->launches += 1;
+}
+
+static lam_status init_host_path(lam_plan* p) {
+  if (p->host_path_ready) return LAM_OK;
+  const size_t esz = p->prm.input == LAM_INPUT_U16_RAW ? 2 : 4;
+  p->ZR = (int)std::max<size_t>(1, std::min<size_t>(p->n, (64u << 20) / ((size_t)p->nz * p->n * 4)));
+  while (p->n % p->ZR) --p->ZR;
+  lam_status st;
+  for (int i = 0; i < 2; ++i) {
+    char* q = nullptr;
+    if ((st = dalloc(p, &q, (size_t)p->TC * p->h * p->w * esz)) != LAM_OK) return st;
+    p->d_in[i] = q;
+    if ((st = dalloc(p, &p->d_out[i], (size_t)p->nz * p->ZR * p->n)) != LAM_OK) return st;
+    CU(p, cudaEventCreateWithFlags(&p->ev_in_ready[i], cudaEventDisableTiming));
+    CU(p, cudaEventCreateWithFlags(&p->ev_in_free[i], cudaEventDisableTiming));
+    CU(p, cudaEventCreateWithFlags(&p->ev_out_ready[i], cudaEventDisableTiming));
+    CU(p, cudaEventCreateWithFlags(&p->ev_out_free[i], cudaEventDisableTiming));
+  }
+  CU(p, cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming));
+  CU(p, cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
+  CU(p, cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
+  p->host_path_ready = true;
+  return LAM_OK;
 }
 
 lam_status lam_backproject(lam_plan* p, const void* proj, float* vol, void* cuda_stream) {
@@ -553,26 +595,71 @@ lam_status lam_backproject(lam_plan* p, const void* proj, float* vol, void* cuda
   if (p->prm.input == LAM_INPUT_U16_RAW && !p->have_darkflat) return fail(p, LAM_EINVAL, "uint16 input needs lam_set_darkflat first");
   cudaSetDevice(p->device);
   cudaStream_t s = (cudaStream_t)cuda_stream;
-  if (!is_device_ptr(proj) || !is_device_ptr(vol))
-    return fail(p, LAM_EUNSUPPORTED, "host-pointer (out-of-core) path is not implemented in this build");
+  const bool proj_dev = is_device_ptr(proj), vol_dev = is_device_ptr(vol);
+  if (!proj_dev || !vol_dev) {
+    lam_status st = init_host_path(p);
+    if (st != LAM_OK) return st;
+  }
   p->launches = 0;
   p->events_used = 0;
   p->stage_valid = false;
   const size_t esz = p->prm.input == LAM_INPUT_U16_RAW ? 2 : 4;
+  const size_t pbytes = (size_t)p->h * p->w * esz;
   {
     StageScope total(p, 5, s);
-    {
+    if (proj_dev) {
       StageScope sc(p, 0, s);
       for (int th0 = 0; th0 < p->ntheta; th0 += p->TC) {
         int nth = std::min(p->TC, p->ntheta - th0);
-        launch_s1(p, (const char*)proj + (size_t)th0 * p->h * p->w * esz, th0, nth, s);
+        launch_s1(p, (const char*)proj + (size_t)th0 * pbytes, th0, nth, s);
+      }
+    } else {
+      // projections stream host -> device in chunks on the copy stream, double-buffered against S0+S1
+      CU(p, cudaEventRecord(p->ev_fork, s));
+      CU(p, cudaStreamWaitEvent(p->s_h2d, p->ev_fork, 0));
+      int c = 0;
+      for (int th0 = 0; th0 < p->ntheta; th0 += p->TC, ++c) {
+        int nth = std::min(p->TC, p->ntheta - th0), b = c & 1;
+        if (c >= 2) CU(p, cudaStreamWaitEvent(p->s_h2d, p->ev_in_free[b], 0));
+        {
+          StageScope sc(p, 4, p->s_h2d);
+          CU(p, cudaMemcpyAsync(p->d_in[b], (const char*)proj + (size_t)th0 * pbytes, (size_t)nth * pbytes, cudaMemcpyHostToDevice, p->s_h2d));
+        }
+        CU(p, cudaEventRecord(p->ev_in_ready[b], p->s_h2d));
+        CU(p, cudaStreamWaitEvent(s, p->ev_in_ready[b], 0));
+        {
+          StageScope sc(p, 0, s);
+          launch_s1(p, p->d_in[b], th0, nth, s);
+        }
+        CU(p, cudaEventRecord(p->ev_in_free[b], s));
       }
     }
     for (int p0 = 0; p0 < p->NP; p0 += p->PB) launch_planes(p, p0, std::min(p->PB, p->NP - p0), s);
-    launch_z(p, vol, s);
+    if (vol_dev) {
+      launch_z(p, vol, (size_t)p->n * p->n, 0, p->n, 0, s);
+    } else {
+      // volume leaves in slabs of ZR x2-rows, double-buffered against the x3 stage
+      int c = 0;
+      for (int r0 = 0; r0 < p->n; r0 += p->ZR, ++c) {
+        int b = c & 1;
+        if (c >= 2) CU(p, cudaStreamWaitEvent(s, p->ev_out_free[b], 0));
+        launch_z(p, p->d_out[b], (size_t)p->ZR * p->n, r0, p->ZR, r0, s);
+        CU(p, cudaEventRecord(p->ev_out_ready[b], s));
+        CU(p, cudaStreamWaitEvent(p->s_d2h, p->ev_out_ready[b], 0));
+        {
+          StageScope sc(p, 4, p->s_d2h);
+          CU(p, cudaMemcpy2DAsync(vol + (size_t)r0 * p->n, (size_t)p->n * p->n * 4, p->d_out[b], (size_t)p->ZR * p->n * 4,
+                                  (size_t)p->ZR * p->n * 4, p->nz, cudaMemcpyDeviceToHost, p->s_d2h));
+        }
+        CU(p, cudaEventRecord(p->ev_out_free[b], p->s_d2h));
+      }
+      CU(p, cudaEventRecord(p->ev_fork, p->s_d2h));
+      CU(p, cudaStreamWaitEvent(s, p->ev_fork, 0));  // join: the user stream completes after the last copy
+    }
   }
   CU(p, cudaGetLastError());
   p->stage_valid = p->profiling;
+  if (!vol_dev) CU(p, cudaStreamSynchronize(p->s_d2h));  // host results are valid on return
   return LAM_OK;
 }
 
