@@ -126,3 +126,191 @@ def cpu_sample(cfg, d, nangles, nslices=1):
     return {"seconds": dt, "value": cfg.voxels * frac / dt / 1e9, "cores": O.threads(),
             "sample": f"{nslices} of {cfg.nz} x3-slices x {len(idx)} of {cfg.ntheta} angles through oracle path C' "
                       f"(fp64 exact-x3 + 2-D gridded USFFT); GVoxel/s scaled by both fractions (cost is linear in each)"}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2401_11101_b200 import inputs, lam
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; this library has no CPU path")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg = inputs.config(args.config)
+    d = inputs.projections(cfg, device="cuda")
+    proj = d["proj"]
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
+                    input="u16" if cfg.raw16 else "f32")
+    if cfg.raw16:
+        plan.set_darkflat(d["dark"], d["flat"])
+    vol = torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        plan.backproject(proj, vol)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    # ---- timed region: K whole back-projections, device-resident input/output, CUDA events on the launching stream
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        plan.backproject(proj, vol)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = plan.info()["launches"] * args.steps
+    # ---- per-stage device times, live, over the same K steps again (events inside the plan; not the headline number)
+    plan.set_profiling(True)
+    stage = [0.0] * 6
+    for _ in range(args.steps):
+        plan.backproject(proj, vol)
+        stage = [a + b for a, b in zip(stage, plan.stage_ms())]
+    plan.set_profiling(False)
+    stage = [s / args.steps for s in stage]
+    clocks = sampler.stop() if rank == 0 else None
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    ms_step = ms / args.steps
+    value = world * cfg.voxels / (ms_step * 1e-3) / 1e9
+
+    # ---- e2e: the same call with host (pinned) buffers; H2D + D2H inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hproj = torch.empty(proj.shape, dtype=proj.dtype, pin_memory=True)
+        hproj.copy_(proj)
+        hvol = torch.empty(vol.shape, dtype=torch.float32, pin_memory=True)
+        for _ in range(2):
+            lam.lam_backproject(plan._plan, hproj.data_ptr(), hvol.data_ptr(), stream.cuda_stream)
+        barrier()
+        ksteps = max(1, min(args.steps, 5))
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for _ in range(ksteps):
+            lam.lam_backproject(plan._plan, hproj.data_ptr(), hvol.data_ptr(), stream.cuda_stream)
+        e1.record(stream)
+        barrier()
+        wall = (time.perf_counter() - t0) * 1e3
+        ems = max(e0.elapsed_time(e1), wall if world == 1 else 0.0)
+        t = torch.tensor([ems], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ems = float(t.item()) / ksteps
+        err = float((hvol.cuda() - vol).norm() / vol.norm())
+        e2e = {"value": world * cfg.voxels / (ems * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ems, "steps": ksteps,
+               "h2d_bytes_per_step": hproj.numel() * hproj.element_size(),
+               "d2h_bytes_per_step": hvol.numel() * 4, "host_vs_device_result_rel_l2": err}
+        del hproj, hvol
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    # ---- rooflines
+    hbm, src = peaks()
+    model = stage_model(cfg)
+    names = list(model.keys())
+    stages = {}
+    for i, nm in enumerate(names):
+        gbs = model[nm]["bytes"] / (stage[i] * 1e-3) / 1e9 if stage[i] > 0 else None
+        stages[nm] = {"ms": round(stage[i], 4), "algorithmic_GB": round(model[nm]["bytes"] / 1e9, 4),
+                      "achieved_GBs": round(gbs, 1) if gbs else None, "hbm_frac": round(gbs / hbm, 4) if gbs else None}
+    dom = max(range(4), key=lambda i: stage[i])
+    if names[dom] == "s2_gridding_xy":
+        peak = 148 * 128 * 2 * 1.965e9 / 1e12   # fp32 FMA lanes x 2 flop x max SM clock
+        ach = model[names[dom]]["flops"] / (stage[dom] * 1e-3) / 1e12
+        roof = {"kernel": "k_spread (+k_zero_tiles)", "stage": names[dom], "bound": "alu", "achieved": round(ach, 3),
+                "peak": round(peak, 2), "unit": "TFLOP/s", "frac": round(ach / peak, 4), "traffic": None,
+                "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 flop x 1.965 GHz"}
+    else:
+        ach = model[names[dom]]["bytes"] / (stage[dom] * 1e-3) / 1e9
+        roof = {"kernel": names[dom], "stage": names[dom], "bound": "hbm", "achieved": round(ach, 1), "peak": hbm,
+                "unit": "GB/s", "frac": round(ach / hbm, 4), "traffic": None, "peak_source": src}
+    roof["stages"] = stages
+    roof["share_of_step"] = round(stage[dom] / max(1e-9, sum(stage[:4])), 4)
+    total_bytes = sum(m["bytes"] for m in model.values())
+    roof["whole_step_hbm_frac"] = round(total_bytes / (ms_step * 1e-3) / 1e9 / hbm, 4)
+    out = {"metric": METRIC, "value": round(value, 4), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 4), "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": f"configs[{args.config}] {cfg.name}: volume {cfg.n}x{cfg.n}x{cfg.nz} fp32, "
+                                  f"{cfg.ntheta} angles, phi={cfg.phi_deg} deg, detector {cfg.h}x{cfg.w} "
+                                  f"{'uint16 raw + dark/flat' if cfg.raw16 else 'fp32'}, KB W={cfg.width} sigma={cfg.oversample}",
+                      "l2": "inputs larger than L2 (projections %.2f GB, spectra %.2f GB per step)" % (
+                          proj.numel() * proj.element_size() / 1e9, model["s2_gridding_xy"]["bytes"] / 1e9),
+                      "parallelism": "replicas only" if world > 1 else "single GPU",
+                      "plan": plan.info()},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof}
+    if not args.no_cpu_baseline:
+        na = args.cpu_angles or max(1, min(cfg.ntheta, int(round(32 * (256 * 256) / (cfg.h * cfg.w)))))
+        cb = cpu_sample(cfg, d, na)
+        out["cpu_baseline"] = {"value": float(f"{cb['value']:.6g}"), "unit": UNIT, "cores": cb["cores"], "kind": "oracle",
+                               "sample": cb["sample"], "seconds": round(cb["seconds"], 2)}
+    print(json.dumps(out), flush=True)
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_reference(args):
+    """The reference arm of this tier = the CPU oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2401_11101_b200 import inputs
+    cfg = inputs.config(args.config)
+    import torch
+    na = args.cpu_angles or max(1, min(cfg.ntheta, int(round(8 * (256 * 256) / (cfg.h * cfg.w)))))
+    # only the sampled angles are generated (same recipe, same seed; the angle subset is part of the stated sample)
+    step = max(1, cfg.ntheta // na)
+    import numpy as np
+    idx = np.arange(0, cfg.ntheta, step)[:na]
+    dev = "cuda" if torch.cuda.is_available() else "cpu"
+    d = inputs.projections(cfg, device=dev, theta=cfg.theta()[idx])
+    d = {k: (v.cpu() if hasattr(v, "cpu") else v) for k, v in d.items()}
+    from oracle import lam_oracle as O
+    dark = d["dark"].numpy() if d["dark"] is not None else None
+    flat = d["flat"].numpy() if d["flat"] is not None else None
+    g = O.Geometry(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, dark=dark, flat=flat)
+    proj = d["proj"].contiguous().numpy()
+    times = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        O.fbp_gridded_slice(g, proj, cfg.nz // 2, W=cfg.width, sigma=cfg.oversample)
+        dt = time.perf_counter() - t0
+        if it >= args.warmup:
+            times.append(dt)
+    dt = sum(times) / len(times)
+    frac = (1.0 / cfg.nz) * (len(idx) / cfg.ntheta)
+    value = cfg.voxels * frac / dt / 1e9
+    sample = (f"per step: 1 of {cfg.nz} x3-slices x {len(idx)} of {cfg.ntheta} angles through oracle path C' (fp64); "
+              f"GVoxel/s scaled by both fractions (cost is linear in each)")
+    out = {"impl": "reference", "metric": METRIC, "value": float(f"{value:.6g}"), "unit": UNIT,
+           "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": round(dt * 1e3, 2), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"configs[{args.config}] {cfg.name} (bounded sample, see cpu_baseline.sample)"},
+           "cpu_baseline": {"value": float(f"{value:.6g}"), "unit": UNIT, "cores": O.threads(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": float(f"{value:.6g}"), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -154,36 +154,40 @@ def detector_fields(cfg, device="cpu"):
     return dark.float().to(device), flat.float().to(device)
 
 
-def projections(cfg, device="cpu", out=None, chunk=None):
+def projections(cfg, device="cpu", out=None, chunk=None, theta=None):
     """Full input of a config.
 
     Returns dict(proj=..., dark=..., flat=..., theta=float64 numpy):
       fp32 configs : proj float32 [ntheta][h][w] line integrals (+ noise for configs[1])
       raw16 configs: proj uint16 counts, dark/flat float32 [h][w]
-    `out` may be a preallocated tensor (e.g. pinned host memory for the out-of-core config)."""
+    `out` may be a preallocated tensor (e.g. pinned host memory for the out-of-core config).
+    `theta` (optional): generate only these angles (a bounded sample of the scan; global scales are still taken
+    from the full angle set, the noise stream is the sample's own)."""
     device = torch.device(device)
     dtype = torch.float64 if device.type == "cpu" else torch.float32
     ph = phantom(cfg)
-    theta = cfg.theta()
+    full_theta = cfg.theta()
+    theta = full_theta if theta is None else np.ascontiguousarray(theta, dtype=np.float64)
+    ntheta = len(theta)
     if chunk is None:
         chunk = max(1, int(2 ** 26 // max(1, cfg.nblobs * max(cfg.h, cfg.w) + cfg.h * cfg.w * 8)))
     odt = torch.uint16 if cfg.raw16 else torch.float32
     if out is None:
-        out = torch.empty((cfg.ntheta, cfg.h, cfg.w), dtype=odt, device=device)
+        out = torch.empty((ntheta, cfg.h, cfg.w), dtype=odt, device=device)
     dark = flat = None
     scale = 1.0
     if cfg.raw16:
         dark, flat = detector_fields(cfg, device)
         # one global scale so that max d = dmax (transmission >= 15 %, PAPER.md:234); found on a theta subset
-        sub = theta[:: max(1, cfg.ntheta // 16)]
+        sub = full_theta[:: max(1, cfg.ntheta // 16)]
         scale = cfg.dmax / float(_line_integrals(cfg, ph, sub, device, dtype).max())
     gen = torch.Generator(device=device).manual_seed(cfg.seed + 104729)
     dmax = None
     if cfg.noise > 0:
-        sub = theta[:: max(1, cfg.ntheta // 16)]
+        sub = full_theta[:: max(1, cfg.ntheta // 16)]
         dmax = float(_line_integrals(cfg, ph, sub, device, dtype).max())
-    for t0 in range(0, cfg.ntheta, chunk):
-        t1 = min(cfg.ntheta, t0 + chunk)
+    for t0 in range(0, ntheta, chunk):
+        t1 = min(ntheta, t0 + chunk)
         d = _line_integrals(cfg, ph, theta[t0:t1], device, dtype) * scale
         if cfg.noise > 0:
             d = d + cfg.noise * dmax * torch.randn(d.shape, generator=gen, device=device, dtype=dtype)
