@@ -23,8 +23,9 @@ def rel(a, b):
 
 
 def run_gpu(cfg, d, **kw):
-    plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
-                    input="u16" if cfg.raw16 else "f32", **kw)
+    args = dict(nz=cfg.nz, width=cfg.width, oversample=cfg.oversample, input="u16" if cfg.raw16 else "f32")
+    args.update(kw)
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, **args)
     if cfg.raw16:
         plan.set_darkflat(d["dark"].cuda(), d["flat"].cuda())
     vol = plan.backproject(d["proj"].cuda())
