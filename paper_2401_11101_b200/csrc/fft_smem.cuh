@@ -1,15 +1,20 @@
-// fft_smem.cuh — batched power-of-two complex FFT inside one thread block, in shared memory.
+// fft_smem.cuh — batched power-of-two complex FFT inside one thread block: radix stages in registers, the
+// exchanges between stages through shared memory.
 //
 // Used by every FFT pass of the path: F_2D of Eq. 7 on the projections and the inverse FFT of the
 // USFFT ("second step is replaced to inverse 3D FFT") along x1, x2 and x3.
 //
-// Algorithm: in-place decimation-in-frequency, ceil(log2 N / 4) passes of radix 4..16.  In a pass every work item
-// holds R = 2^rb elements (stride S) in registers, runs a radix-R butterfly there, applies the inter-pass twiddles
-// and writes back to the same addresses.  The result is left in (mixed-radix) digit-reversed order; consumers read
-// X[k] at fft_pos<LOGN>(k), so the permutation costs nothing.  Shared-memory index i is stored at i + i/16
-// (fft_phys) which keeps both the stride-S reads of early passes and the stride-1 groups of the last pass free of
-// bank conflicts for 8-byte elements.  Twiddles: one table lookup e^{-2 pi i j/L} per work item (table computed in
-// double on the host), its powers by at most log-depth complex products.
+// Algorithm: decimation in frequency in ceil(log2 N / 4) passes of radix 4..16.  Pass 0 takes its inputs straight
+// from a caller-supplied loader (global memory, coalesced: work item u reads elements u + k*S0), every pass runs a
+// radix-R butterfly in registers and applies the inter-pass twiddles, passes exchange through shared memory
+// in place, and the last pass hands its outputs to a caller-supplied sink (global memory, coalesced: work item v
+// holds the bins v + q*N/R_last) or leaves them in shared memory for an epilogue that needs other bins.
+// The data in shared memory is in mixed-radix digit-reversed order; bin k lives at fft_at<LOGN>(k).
+// Shared-memory position p is stored at fft_swz<LOGN>(p): an XOR of the low four position bits with the
+// bit-reversed leading digit (and one bit of the second digit for four-pass sizes), which makes every access
+// pattern of every pass (16 lanes of a half-warp, 8-byte elements) hit 16 distinct banks; two-pass sizes
+// (N <= 256) use the additive padding p + p/16 instead.  Twiddles: one table lookup e^{-2 pi i j/L} per work item
+// (table computed in double on the host), its powers by at most log-depth complex products.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -20,9 +25,6 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
 }
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-
-__host__ __device__ constexpr int fft_phys(int i) { return i + (i >> 4); }
-__host__ __device__ constexpr int fft_pitch(int n) { return n + (n >> 4); }
 
 template <int LOGN>
 struct FftShape {
@@ -35,7 +37,28 @@ struct FftShape {
   }
 };
 
-// position (logical, before fft_phys) of output bin k after all passes
+// elements of shared memory one transform of length n occupies (before the caller's own row padding)
+__host__ __device__ constexpr int fft_span(int n) { return n <= 256 ? n + (n >> 4) : n; }
+
+// shared-memory pitch of a TFAST block_fft: a multiple of 16 plus 16/nb (nb <= 16 transforms) or 1
+__host__ __device__ constexpr int fft_tfast_pitch(int n, int nb) { return ((fft_span(n) + 15) & ~15) + (nb >= 16 ? 1 : 16 / nb); }
+
+// physical index of logical position p of a transform
+template <int LOGN>
+__device__ __forceinline__ int fft_swz(int p) {
+  using F = FftShape<LOGN>;
+  if constexpr (F::NP <= 2) {
+    return p + (p >> 4);
+  } else {
+    const int d0 = p >> F::sb(0);
+    int x = (int)(__brev((unsigned)d0) >> 28);
+    if constexpr (F::rb(0) == 3) x ^= d0 & 1;
+    if constexpr (F::NP == 4) x ^= ((p >> F::sb(1)) & 1) << 3;
+    return p ^ x;
+  }
+}
+
+// logical position of output bin k after all passes (mixed-radix digit reversal)
 template <int LOGN>
 __device__ __forceinline__ int fft_pos(int k) {
   using F = FftShape<LOGN>;
@@ -46,6 +69,10 @@ __device__ __forceinline__ int fft_pos(int k) {
     sh += F::rb(i);
   }
   return p;
+}
+template <int LOGN>
+__device__ __forceinline__ int fft_at(int k) {
+  return fft_swz<LOGN>(fft_pos<LOGN>(k));
 }
 
 // d * e^{DIR * 2 pi i k16 / 16}, k16 a compile-time constant after unrolling
@@ -84,18 +111,14 @@ __device__ __forceinline__ void fft_reg(float2 (&a)[R]) {
   }
 }
 
-// one work item of pass I on one transform s[] (logical indexing through fft_phys)
+// butterfly of pass I on registers a[k] = x[base + k*S] (j = index inside the stride) followed by the inter-pass
+// twiddles; on return a[brev(q)] is output digit q
 template <int LOGN, int DIR, int I>
-__device__ __forceinline__ void fft_pass_item(float2* s, int u, const float2* __restrict__ tw) {
+__device__ __forceinline__ void fft_bfly(float2 (&a)[1 << FftShape<LOGN>::rb(I)], int j, const float2* __restrict__ tw) {
   using F = FftShape<LOGN>;
-  constexpr int RB = F::rb(I), R = 1 << RB, SB = F::sb(I), S = 1 << SB;
-  const int j = u & (S - 1);
-  const int base = ((u >> SB) << (SB + RB)) | j;
-  float2 a[R];
-#pragma unroll
-  for (int k = 0; k < R; ++k) a[k] = s[fft_phys(base + k * S)];
+  constexpr int RB = F::rb(I), R = 1 << RB, SB = F::sb(I);
   fft_reg<R, DIR>(a);
-  if (SB > 0) {
+  if constexpr (SB > 0) {
     float2 w[R];
     w[1] = __ldg(&tw[j << (LOGN - SB - RB)]);  // e^{-2 pi i j / L}, L = R*S
     if (DIR > 0) w[1].y = -w[1].y;
@@ -104,29 +127,100 @@ __device__ __forceinline__ void fft_pass_item(float2* s, int u, const float2* __
 #pragma unroll
     for (int q = 1; q < R; ++q) a[brev_bits(q, RB)] = cmul(a[brev_bits(q, RB)], w[q]);
   }
-#pragma unroll
-  for (int q = 0; q < R; ++q) s[fft_phys(base + q * S)] = a[brev_bits(q, RB)];
 }
 
-template <int LOGN, int DIR, int I>
-__device__ __forceinline__ void fft_passes(float2* s, int nb, int pitch, const float2* __restrict__ tw) {
-  using F = FftShape<LOGN>;
-  if constexpr (I < F::NP) {
-    constexpr int IB = LOGN - F::rb(I);  // log2(items per transform)
-    const int total = nb << IB;
-    for (int it = threadIdx.x; it < total; it += blockDim.x)
-      fft_pass_item<LOGN, DIR, I>(s + (it >> IB) * pitch, it & ((1 << IB) - 1), tw);
-    __syncthreads();
-    fft_passes<LOGN, DIR, I + 1>(s, nb, pitch, tw);
+// work item -> (transform t, item u).  TFAST: consecutive threads take consecutive transforms (column FFTs whose
+// transforms are adjacent in global memory; nb = 1 << lognb); otherwise consecutive threads take consecutive items.
+template <bool TFAST>
+__device__ __forceinline__ void fft_split(int it, int itembits, int lognb, int& t, int& u) {
+  if (TFAST) {
+    t = it & ((1 << lognb) - 1);
+    u = it >> lognb;
+  } else {
+    t = it >> itembits;
+    u = it & ((1 << itembits) - 1);
   }
 }
 
-// nb transforms of length 2^LOGN, transform t at s + t*pitch (pitch >= fft_pitch(N)), element i at fft_phys(i).
+template <int LOGN, int DIR, bool TFAST, int I>
+__device__ __forceinline__ void fft_mid_passes(float2* s, int nb, int lognb, int pitch, const float2* __restrict__ tw) {
+  using F = FftShape<LOGN>;
+  if constexpr (I < F::NP - 1) {
+    constexpr int RB = F::rb(I), R = 1 << RB, SB = F::sb(I), S = 1 << SB, IB = LOGN - RB;
+    for (int it = threadIdx.x; it < nb << IB; it += blockDim.x) {
+      int t, u;
+      fft_split<TFAST>(it, IB, lognb, t, u);
+      const int j = u & (S - 1), base = ((u >> SB) << (SB + RB)) | j;
+      float2* st = s + t * pitch;
+      float2 a[R];
+#pragma unroll
+      for (int k = 0; k < R; ++k) a[k] = st[fft_swz<LOGN>(base + k * S)];
+      fft_bfly<LOGN, DIR, I>(a, j, tw);
+#pragma unroll
+      for (int q = 0; q < R; ++q) st[fft_swz<LOGN>(base + q * S)] = a[brev_bits(q, RB)];
+    }
+    __syncthreads();
+    fft_mid_passes<LOGN, DIR, TFAST, I + 1>(s, nb, lognb, pitch, tw);
+  }
+}
+
+// nb transforms of length N = 2^LOGN (transform t at s + t*pitch, pitch >= fft_span(N)).
+//   ld(t, i)     -> float2 input element i of transform t           (called once per element, pass 0)
+//   st(t, k, v)  :  output bin k of transform t                     (SINK = true; called once per bin, last pass)
+//   SINK = false :  the outputs stay in shared memory, bin k at s[t*pitch + fft_at<LOGN>(k)]; ends with a barrier.
 // DIR = -1: X[k] = sum x[i] e^{-2 pi i ik/N};  DIR = +1: e^{+...} (unnormalised).  tw: N entries e^{-2 pi i k/N}.
-// Must be called by all threads of the block; ends with a __syncthreads().  Caller syncs after filling s.
-template <int LOGN, int DIR>
-__device__ __forceinline__ void block_fft(float2* s, int nb, int pitch, const float2* __restrict__ tw) {
-  fft_passes<LOGN, DIR, 0>(s, nb, pitch, tw);
+// Must be called by all threads of the block.  In TFAST mode nb = 1 << lognb and pitch = fft_tfast_pitch(N, nb)
+// (a multiple of 16 plus 16/nb) makes every access conflict-free; otherwise lognb is ignored.
+template <int LOGN, int DIR, bool TFAST, bool SINK, class LD, class ST>
+__device__ __forceinline__ void block_fft(float2* s, int nb, int lognb, int pitch, const float2* __restrict__ tw, LD ld, ST st) {
+  using F = FftShape<LOGN>;
+  {  // pass 0: global -> registers -> shared
+    constexpr int RB = F::rb(0), R = 1 << RB, SB = F::sb(0), S = 1 << SB, IB = LOGN - RB;
+    for (int it = threadIdx.x; it < nb << IB; it += blockDim.x) {
+      int t, u;
+      fft_split<TFAST>(it, IB, lognb, t, u);
+      float2 a[R];
+#pragma unroll
+      for (int k = 0; k < R; ++k) a[k] = ld(t, u + k * S);
+      fft_bfly<LOGN, DIR, 0>(a, u, tw);
+      float2* sp = s + t * pitch;
+#pragma unroll
+      for (int q = 0; q < R; ++q) sp[fft_swz<LOGN>(u + q * S)] = a[brev_bits(q, RB)];
+    }
+    __syncthreads();
+  }
+  fft_mid_passes<LOGN, DIR, TFAST, 1>(s, nb, lognb, pitch, tw);
+  {  // last pass: shared -> registers -> sink (or back in place)
+    constexpr int I = F::NP - 1, RB = F::rb(I), R = 1 << RB, IB = LOGN - RB;
+    for (int it = threadIdx.x; it < nb << IB; it += blockDim.x) {
+      int t, e;
+      fft_split<TFAST>(it, IB, lognb, t, e);
+      // item v holds the bins v + q*2^IB.  In TFAST mode with nb < 16 transforms a half-warp holds 16/nb items:
+      // enumerate them with the low four bits reversed, so that consecutive items differ in the high bits of the
+      // leading digit = the low bits of the swizzled bank.
+      int v = e;
+      if (TFAST && F::rb(0) == 4 && IB >= 4) v = (e & ~15) | (int)(__brev((unsigned)e) >> 28);
+      int base = 0, sh = 0;
+#pragma unroll
+      for (int i = 0; i < I; ++i) {
+        base |= ((v >> sh) & ((1 << F::rb(i)) - 1)) << F::sb(i);
+        sh += F::rb(i);
+      }
+      float2* sp = s + t * pitch;
+      float2 a[R];
+#pragma unroll
+      for (int k = 0; k < R; ++k) a[k] = sp[fft_swz<LOGN>(base + k)];
+      fft_reg<R, DIR>(a);
+      if constexpr (SINK) {
+#pragma unroll
+        for (int q = 0; q < R; ++q) st(t, v + (q << IB), a[brev_bits(q, RB)]);
+      } else {
+#pragma unroll
+        for (int q = 0; q < R; ++q) sp[fft_swz<LOGN>(base + q)] = a[brev_bits(q, RB)];
+      }
+    }
+    if constexpr (!SINK) __syncthreads();
+  }
 }
 
 }  // namespace lam

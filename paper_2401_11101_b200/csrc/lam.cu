@@ -42,7 +42,7 @@ struct lam_plan {
   int M = 0, M3 = 0, W = 0, NP = 0, WR = 0, WQ = 0;
   int logw = 0, logh = 0, logM = 0, logM3 = 0;
   int PB = 1, TC = 1;  // plane batch, theta chunk
-  int rows_nb = 1, cols_cb = 1, x1_nb = 1, x2_nb = 1, z_cb = 1;
+  int rows_nb = 1, cols_lcb = 3, x1_nb = 1, x2_lnb = 3, KZ = 1;
   GridKernel gk;
   KerPoly kp{};
   SpreadGeom geom{};
@@ -50,9 +50,8 @@ struct lam_plan {
   double2* d_cs = nullptr;
   float2 *d_Pu = nullptr, *d_Pv = nullptr, *d_PuNone = nullptr;
   float2 *d_tw_w = nullptr, *d_tw_h = nullptr, *d_tw_M = nullptr, *d_tw_M3 = nullptr;
-  float *d_wz = nullptr, *d_dx = nullptr, *d_dz = nullptr, *d_dark = nullptr, *d_flat = nullptr;
-  int* d_bz = nullptr;
-  int2* d_prange = nullptr;
+  float *d_ztab = nullptr, *d_zlast = nullptr, *d_dx = nullptr, *d_dz = nullptr, *d_dark = nullptr, *d_flat = nullptr;
+  int* d_zlo = nullptr;
   uint2* d_jobs = nullptr;
   std::vector<long long> job_off;  // [NP+1] first job of each plane
   // workspace
@@ -149,17 +148,17 @@ struct Launch {
       k_rows<L, false><<<g, 256, sm, s>>>(a);
     }
   }
-  static void cols(dim3 g, size_t sm, cudaStream_t s, const ColsArgs& a) {
+  static void cols(dim3 g, int threads, size_t sm, cudaStream_t s, const ColsArgs& a) {
     cudaFuncSetAttribute(k_cols<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    k_cols<L><<<g, 256, sm, s>>>(a);
+    k_cols<L><<<g, threads, sm, s>>>(a);
   }
   static void x1(dim3 g, size_t sm, cudaStream_t s, const IfftArgs& a) {
     cudaFuncSetAttribute(k_ifft_x1<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     k_ifft_x1<L><<<g, 256, sm, s>>>(a);
   }
-  static void x2(dim3 g, size_t sm, cudaStream_t s, const IfftArgs& a) {
+  static void x2(dim3 g, int threads, size_t sm, cudaStream_t s, const IfftArgs& a) {
     cudaFuncSetAttribute(k_ifft_x2<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    k_ifft_x2<L><<<g, 256, sm, s>>>(a);
+    k_ifft_x2<L><<<g, threads, sm, s>>>(a);
   }
   static void z(dim3 g, size_t sm, cudaStream_t s, const ZArgs& a) {
     cudaFuncSetAttribute(k_zstage<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
@@ -207,7 +206,7 @@ struct StageScope {
 
 void free_all(lam_plan* p) {
   void* ptrs[] = {p->d_cs,    p->d_Pu,  p->d_Pv,  p->d_PuNone, p->d_tw_w, p->d_tw_h,   p->d_tw_M, p->d_tw_M3,
-                  p->d_wz,    p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_bz,     p->d_prange, p->d_jobs,
+                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs,
                   p->d_R,     p->d_S,   p->d_G,   p->d_T,      p->d_A};
   for (void* q : ptrs)
     if (q) cudaFree(q);
@@ -321,26 +320,40 @@ lam_status make_tables(lam_plan* p) {
   // gridding kernel: polynomial pieces for (xi1, xi2); explicit weights for xi3 (they depend on k_v only)
   p->gk.init(p->prm.kernel, W, sigma, p->prm.shape);
   kernel_poly(p->gk, &p->kp.E[0][0], &p->kp.O[0][0]);
-  std::vector<float> wz((size_t)NP * W);
-  std::vector<int> bz(NP);
-  std::vector<int2> prange(M3, make_int2(1, 0));
-  const double cphi = std::cos(p->phi);
-  for (int q = 0; q < NP; ++q) {
-    int kv = q == h / 2 ? -h / 2 : q;
-    double t3 = (double)M3 * kv * cphi / h;
-    int b = (int)std::ceil(t3 - 0.5 * W);
-    bz[q] = b;
-    for (int j = 0; j < W; ++j) wz[(size_t)q * W + j] = (float)p->gk.kap(t3 - (b + j));
-    if (q < h / 2)
+  // x3 gridding as a banded matrix: for grid cell i (stored index m3 mod M3) the planes p < h/2 with a tap on it
+  // are contiguous; the k_v = -h/2 plane (p = h/2) is kept apart
+  {
+    const double cphi = std::cos(p->phi);
+    std::vector<int> lo(M3, 0), hi(M3, -1);
+    auto cell = [&](int m) { return ((m % M3) + M3) % M3; };
+    for (int q = 0; q < h / 2; ++q) {
+      double t3 = (double)M3 * q * cphi / h;
+      int b = (int)std::ceil(t3 - 0.5 * W);
       for (int j = 0; j < W; ++j) {
-        int i = ((b + j) % M3 + M3) % M3;
-        if (prange[i].x > prange[i].y) prange[i] = make_int2(q, q);
-        else { prange[i].x = std::min(prange[i].x, q); prange[i].y = std::max(prange[i].y, q); }
+        int i = cell(b + j);
+        if (hi[i] < lo[i]) lo[i] = hi[i] = q;
+        else { lo[i] = std::min(lo[i], q); hi[i] = std::max(hi[i], q); }
       }
+    }
+    int KZ = 1;
+    for (int i = 0; i < M3; ++i) KZ = std::max(KZ, hi[i] - lo[i] + 1);
+    p->KZ = KZ;
+    std::vector<float> ztab((size_t)M3 * KZ, 0.f), zlast(M3, 0.f);
+    for (int q = 0; q <= h / 2; ++q) {
+      int kv = q == h / 2 ? -h / 2 : q;
+      double t3 = (double)M3 * kv * cphi / h;
+      int b = (int)std::ceil(t3 - 0.5 * W);
+      for (int j = 0; j < W; ++j) {
+        int i = cell(b + j);
+        float wv = (float)p->gk.kap(t3 - (b + j));
+        if (q == h / 2) zlast[i] += wv;
+        else ztab[(size_t)i * KZ + (q - lo[i])] += wv;
+      }
+    }
+    if ((st = upload(p, &p->d_ztab, ztab)) != LAM_OK) return st;
+    if ((st = upload(p, &p->d_zlo, lo)) != LAM_OK) return st;
+    if ((st = upload(p, &p->d_zlast, zlast)) != LAM_OK) return st;
   }
-  if ((st = upload(p, &p->d_wz, wz)) != LAM_OK) return st;
-  if ((st = upload(p, &p->d_bz, bz)) != LAM_OK) return st;
-  if ((st = upload(p, &p->d_prange, prange)) != LAM_OK) return st;
   std::vector<float> dx(n), dz(nz);
   for (int i = 0; i < n; ++i) dx[i] = (float)(1.0 / p->gk.kaphat((double)(i - n / 2) / M));
   for (int i = 0; i < nz; ++i) dz[i] = (float)(1.0 / p->gk.kaphat((double)(i - nz / 2) / M3));
@@ -360,7 +373,7 @@ lam_status make_tables(lam_plan* p) {
   return LAM_OK;
 }
 
-size_t zstage_smem(const lam_plan* p, int cb) { return ((size_t)p->NP * cb + (size_t)cb * fft_pitch(p->M3)) * sizeof(float2); }
+size_t zstage_smem(const lam_plan* p) { return ((size_t)(p->NP + p->KZ) * kZCb + (size_t)kZCb * fft_tfast_pitch(p->M3, kZCb)) * sizeof(float2); }
 
 }  // namespace
 
@@ -454,15 +467,12 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
 
   // block shapes
   p->rows_nb = std::min(h / 2, std::max(1, 4096 / w));
-  p->cols_cb = std::max(2, std::min(32, 8192 / h));
   p->x1_nb = std::max(1, std::min(M, 4096 / M));
-  p->x2_nb = std::min(n, std::max(2, std::min(32, 16384 / M)));
-  {
-    int cb = 32;
-    while (cb > 1 && (zstage_smem(p, cb) > 110 * 1024 || n % cb)) cb >>= 1;
-    if (zstage_smem(p, cb) > 220 * 1024) return bail(fail(p, LAM_EUNSUPPORTED, "x3 stage does not fit shared memory (h = %d, sigma*nz = %d)", h, M3));
-    p->z_cb = cb;
-  }
+  auto tfast_lognb = [](int len) { int l = 3; while (l > 0 && (size_t)(1 << l) * fft_tfast_pitch(len, 1 << l) * 8 > 200 * 1024) --l; return l; };
+  p->cols_lcb = tfast_lognb(h);
+  p->x2_lnb = tfast_lognb(M);
+  if (n % 8) return bail(fail(p, LAM_EUNSUPPORTED, "n must be a multiple of 8"));
+  if (zstage_smem(p) > 220 * 1024) return bail(fail(p, LAM_EUNSUPPORTED, "x3 stage does not fit shared memory (h = %d, sigma*nz = %d)", h, M3));
   // workspace: batch sizes from the budget
   size_t freeb = 0, totalb = 0;
   if (cudaMemGetInfo(&freeb, &totalb) != cudaSuccess) return bail(fail(p, LAM_ECUDA, "cudaMemGetInfo failed"));
@@ -524,12 +534,13 @@ static void launch_s1(lam_plan* p, const void* chunk, int th0, int nth, cudaStre
   const bool raw = p->prm.input == LAM_INPUT_U16_RAW;
   RowsArgs ra{chunk, p->d_dark, p->d_flat, p->prm.t_min, p->d_R, p->d_Pu, p->d_tw_w, p->h, p->WR, p->rows_nb};
   dim3 gr(p->h / 2 / p->rows_nb, nth);
-  size_t smr = (size_t)p->rows_nb * fft_pitch(p->w) * sizeof(float2);
+  size_t smr = (size_t)p->rows_nb * fft_span(p->w) * sizeof(float2);
   DISPATCH_LOG(p->logw, rows(raw, gr, smr, s, ra));
-  ColsArgs ca{p->d_R, p->d_S, p->d_Pv, p->d_tw_h, p->w, p->WR, p->WQ, p->ntheta, th0, p->cols_cb};
-  dim3 gc((p->w / 2 + 1 + p->cols_cb - 1) / p->cols_cb, nth);
-  size_t smc = (size_t)p->cols_cb * fft_pitch(p->h) * sizeof(float2);
-  DISPATCH_LOG(p->logh, cols(gc, smc, s, ca));
+  const int cb = 1 << p->cols_lcb;
+  ColsArgs ca{p->d_R, p->d_S, p->d_Pv, p->d_tw_h, p->w, p->WR, p->WQ, p->ntheta, th0, p->cols_lcb};
+  dim3 gc((p->w / 2 + 1 + cb - 1) / cb, nth);
+  size_t smc = (size_t)cb * fft_tfast_pitch(p->h, cb) * sizeof(float2);
+  DISPATCH_LOG(p->logh, cols(gc, (size_t)cb * p->h >= 16384 ? 512 : 256, smc, s, ca));
   p->launches += 2;
 }
 
@@ -549,10 +560,12 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
   }
   {
     StageScope sc(p, 2, s);
-    IfftArgs a1{p->d_G, p->d_T, p->d_tw_M, p->n, p->x1_nb};
-    DISPATCH_LOG(p->logM, x1(dim3(p->M / p->x1_nb, np), (size_t)p->x1_nb * fft_pitch(p->M) * sizeof(float2), s, a1));
-    IfftArgs a2{p->d_T, p->d_A + (size_t)p0 * p->n * p->n, p->d_tw_M, p->n, p->x2_nb};
-    DISPATCH_LOG(p->logM, x2(dim3(p->n / p->x2_nb, np), (size_t)p->x2_nb * fft_pitch(p->M) * sizeof(float2), s, a2));
+    IfftArgs a1{p->d_G, p->d_T, p->d_tw_M, p->n, p->x1_nb, 0};
+    DISPATCH_LOG(p->logM, x1(dim3(p->M / p->x1_nb, np), (size_t)p->x1_nb * fft_span(p->M) * sizeof(float2), s, a1));
+    const int nb2 = 1 << p->x2_lnb;
+    IfftArgs a2{p->d_T, p->d_A + (size_t)p0 * p->n * p->n, p->d_tw_M, p->n, nb2, p->x2_lnb};
+    DISPATCH_LOG(p->logM, x2(dim3(p->n / nb2, np), (size_t)nb2 * p->M >= 16384 ? 512 : 256,
+                             (size_t)nb2 * fft_tfast_pitch(p->M, nb2) * sizeof(float2), s, a2));
   }
   p->launches += 4;
 }
@@ -560,9 +573,9 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
 // x3 stage for x2 rows [x2_0, x2_0 + rows); out holds x2 row `out_x2_0` in its first row, z-stride `zstride` floats
 static void launch_z(lam_plan* p, float* out, size_t zstride, int x2_0, int rows, int out_x2_0, cudaStream_t s) {
   StageScope sc(p, 3, s);
-  ZArgs za{p->d_A, out, zstride, p->d_tw_M3, p->d_wz, p->d_bz, p->d_prange, p->d_dx, p->d_dz,
-           p->n, p->nz, p->NP, p->z_cb, p->W, x2_0, out_x2_0};
-  DISPATCH_LOG(p->logM3, z(dim3(p->n / p->z_cb, rows), zstage_smem(p, p->z_cb), s, za));
+  ZArgs za{p->d_A, out, zstride, p->d_tw_M3, p->d_ztab, p->d_zlo, p->d_zlast, p->d_dx, p->d_dz,
+           p->n, p->nz, p->NP, p->KZ, x2_0, out_x2_0};
+  DISPATCH_LOG(p->logM3, z(dim3(p->n / kZCb, rows), zstage_smem(p), s, za));
   p->launches += 1;
 }
 

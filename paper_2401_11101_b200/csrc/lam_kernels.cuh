@@ -41,35 +41,30 @@ struct RowsArgs {
 
 template <int LOGW, bool RAW>
 __global__ void __launch_bounds__(256) k_rows(RowsArgs a) {
-  constexpr int w = 1 << LOGW, P = fft_pitch(w);
+  constexpr int w = 1 << LOGW, P = fft_span(w);
   extern __shared__ float2 sm[];
   const int th = blockIdx.y, pair0 = blockIdx.x * a.nb;
   const size_t pbase = (size_t)th * a.h * w;
-  for (int idx = threadIdx.x; idx < a.nb << LOGW; idx += blockDim.x) {
-    int t = idx >> LOGW, ju = idx & (w - 1), jv = 2 * (pair0 + t);
-    float x0, x1;
+  auto ld = [&](int t, int ju) -> float2 {
+    const int jv = 2 * (pair0 + t);
     if (RAW) {
       const uint16_t* p = (const uint16_t*)a.proj + pbase + (size_t)jv * w + ju;
       float r0 = (float)p[0], r1 = (float)p[w];
-      float d0 = a.dark[jv * w + ju], d1 = a.dark[(jv + 1) * w + ju];
-      float f0 = a.flat[jv * w + ju], f1 = a.flat[(jv + 1) * w + ju];
+      float d0 = __ldg(&a.dark[jv * w + ju]), d1 = __ldg(&a.dark[(jv + 1) * w + ju]);
+      float f0 = __ldg(&a.flat[jv * w + ju]), f1 = __ldg(&a.flat[(jv + 1) * w + ju]);
       float t0 = (r0 - d0) / fmaxf(f0 - d0, 1.0f), t1 = (r1 - d1) / fmaxf(f1 - d1, 1.0f);
-      x0 = -logf(fmaxf(t0, a.tmin));
-      x1 = -logf(fmaxf(t1, a.tmin));
+      return make_float2(-logf(fmaxf(t0, a.tmin)), -logf(fmaxf(t1, a.tmin)));
     } else {
       const float* p = (const float*)a.proj + pbase + (size_t)jv * w + ju;
-      x0 = p[0];
-      x1 = p[w];
+      return make_float2(p[0], p[w]);
     }
-    sm[t * P + fft_phys(ju)] = make_float2(x0, x1);
-  }
-  __syncthreads();
-  block_fft<LOGW, -1>(sm, a.nb, P, a.tw);
+  };
+  block_fft<LOGW, -1, false, false>(sm, a.nb, 0, P, a.tw, ld, [](int, int, float2) {});
   constexpr int NK = w / 2 + 1;
   for (int idx = threadIdx.x; idx < a.nb * NK; idx += blockDim.x) {
     int t = idx / NK, k = idx - t * NK, jv = 2 * (pair0 + t);
-    float2 zk = sm[t * P + fft_phys(fft_pos<LOGW>(k))];
-    float2 zn = sm[t * P + fft_phys(fft_pos<LOGW>((w - k) & (w - 1)))];
+    float2 zk = sm[t * P + fft_at<LOGW>(k)];
+    float2 zn = sm[t * P + fft_at<LOGW>((w - k) & (w - 1))];
     float2 ra = make_float2(0.5f * (zk.x + zn.x), 0.5f * (zk.y - zn.y));   // spectrum of the even row
     float2 rb = make_float2(0.5f * (zk.y + zn.y), -0.5f * (zk.x - zn.x));  // spectrum of the odd row
     float2 pu = a.Pu[k];
@@ -88,30 +83,26 @@ struct ColsArgs {
   float2* S;         // [h/2+1][ntheta][WQ]
   const float2* Pv;  // [h/2+1]  e^{2 pi i k_v c_v / h}
   const float2* tw;  // length h
-  int w, WR, WQ, ntheta, th0, cb;
+  int w, WR, WQ, ntheta, th0, lcb;  // 1 << lcb columns per block
 };
+
 
 template <int LOGH>
 __global__ void __launch_bounds__(256) k_cols(ColsArgs a) {
-  constexpr int h = 1 << LOGH, P = fft_pitch(h);
+  constexpr int h = 1 << LOGH;
   extern __shared__ float2 sm[];
-  const int thl = blockIdx.y, k0 = blockIdx.x * a.cb;
-  const int nc = min(a.cb, a.w / 2 + 1 - k0);
+  const int kColsLog = a.lcb, kColsCb = 1 << a.lcb, P = fft_tfast_pitch(h, kColsCb);
+  const int thl = blockIdx.y, k0 = blockIdx.x * kColsCb;
+  const int nc = min(kColsCb, a.w / 2 + 1 - k0);
   const float2* Rb = a.R + (size_t)thl * h * a.WR + k0;
-  for (int idx = threadIdx.x; idx < h * a.cb; idx += blockDim.x) {
-    int jv = idx / a.cb, c = idx - jv * a.cb;
-    float2 v = c < nc ? Rb[(size_t)jv * a.WR + c] : make_float2(0.f, 0.f);
-    sm[c * P + fft_phys(jv)] = v;
-  }
-  __syncthreads();
-  block_fft<LOGH, -1>(sm, a.cb, P, a.tw);
+  auto ld = [&](int t, int jv) -> float2 { return t < nc ? Rb[(size_t)jv * a.WR + t] : make_float2(0.f, 0.f); };
+  block_fft<LOGH, -1, true, false>(sm, kColsCb, kColsLog, P, a.tw, ld, [](int, int, float2) {});
   const int hw = a.w / 2, th = a.th0 + thl;
-  for (int idx = threadIdx.x; idx < (h / 2 + 1) * a.cb; idx += blockDim.x) {
-    int p = idx / a.cb, c = idx - p * a.cb;
-    if (c >= nc) continue;
+  auto emit = [&](int p, int c) {
+    if (c >= nc) return;
     int k = k0 + c;
-    float2 cp = sm[c * P + fft_phys(fft_pos<LOGH>(p))];
-    float2 cm = sm[c * P + fft_phys(fft_pos<LOGH>((h - p) & (h - 1)))];
+    float2 cp = sm[c * P + fft_at<LOGH>(p)];
+    float2 cm = sm[c * P + fft_at<LOGH>((h - p) & (h - 1))];
     cm.y = -cm.y;
     float2 pv = a.Pv[p];
     bool mid = p > 0 && p < h / 2;
@@ -121,7 +112,14 @@ __global__ void __launch_bounds__(256) k_cols(ColsArgs a) {
     float2 vp = cmul(cp, pv), vm = cmul(cm, pv);
     Srow[hw + k] = make_float2(vp.x * wplus, vp.y * wplus);
     if (k > 0) Srow[hw - k] = make_float2(vm.x * wminus, vm.y * wminus);
+  };
+  for (int idx = threadIdx.x; idx < (h / 2) * kColsCb; idx += blockDim.x) {
+    int e = idx >> kColsLog, c = idx & (kColsCb - 1);
+    int p = e;  // radix-16 leading digit: low four bits reversed, as in the last FFT pass (distinct banks)
+    if (FftShape<LOGH>::rb(0) == 4 && h / 2 >= 16) p = (e & ~15) | (int)(__brev((unsigned)e) >> 28);
+    emit(p, c);
   }
+  if (threadIdx.x < kColsCb) emit(h / 2, threadIdx.x);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -459,124 +457,111 @@ struct IfftArgs {
   const float2* in;
   float2* out;
   const float2* tw;
-  int n, nb;  // nb: rows (x1 pass) or columns (x2 pass) per block
+  int n, nb, lnb;  // nb = 1 << lnb: rows (x1 pass) or columns (x2 pass) per block
 };
 
 template <int LOGM>
 __global__ void __launch_bounds__(256) k_ifft_x1(IfftArgs a) {
-  constexpr int M = 1 << LOGM, P = fft_pitch(M);
+  constexpr int M = 1 << LOGM, P = fft_span(M);
   extern __shared__ float2 sm[];
   const int pl = blockIdx.y, r0 = blockIdx.x * a.nb;
   const float2* in = a.in + ((size_t)pl * M + r0) * M;
-  for (int idx = threadIdx.x; idx < a.nb << LOGM; idx += blockDim.x) {
-    int t = idx >> LOGM, i = idx & (M - 1);
-    sm[t * P + fft_phys(i)] = in[(size_t)t * M + i];
-  }
-  __syncthreads();
-  block_fft<LOGM, +1>(sm, a.nb, P, a.tw);
   float2* out = a.out + ((size_t)pl * M + r0) * a.n;
-  for (int idx = threadIdx.x; idx < a.nb * a.n; idx += blockDim.x) {
-    int t = idx / a.n, ix = idx - t * a.n, x = ix - a.n / 2;
-    float2 v = sm[t * P + fft_phys(fft_pos<LOGM>(x & (M - 1)))];
-    if (x & 1) { v.x = -v.x; v.y = -v.y; }
-    out[(size_t)t * a.n + ix] = v;
-  }
+  const int n = a.n, hn = a.n / 2;
+  auto ld = [&](int t, int i) -> float2 { return in[(size_t)t * M + i]; };
+  auto st = [&](int t, int k, float2 v) {
+    int ix = k < hn ? k + hn : k - (M - hn);  // x = k (k < n/2) or k - M (k >= M - n/2)
+    if (k >= hn && k < M - hn) return;
+    if (k & 1) { v.x = -v.x; v.y = -v.y; }
+    out[(size_t)t * n + ix] = v;
+  };
+  block_fft<LOGM, +1, false, true>(sm, a.nb, 0, P, a.tw, ld, st);
 }
 
 // S3: inverse FFT along xi2 (columns), cropped:  A[p][ix2][ix1] = (-1)^x2 sum_i2 T[pl][i2][ix1] e^{+2 pi i x2 i2/M}
 template <int LOGM>
-__global__ void __launch_bounds__(256) k_ifft_x2(IfftArgs a) {
-  constexpr int M = 1 << LOGM, P = fft_pitch(M);
+__global__ void __launch_bounds__(512) k_ifft_x2(IfftArgs a) {
+  constexpr int M = 1 << LOGM;
   extern __shared__ float2 sm[];
+  const int P = fft_tfast_pitch(M, a.nb);
   const int pl = blockIdx.y, c0 = blockIdx.x * a.nb;
-  const float2* in = a.in + (size_t)pl * M * a.n + c0;
-  for (int idx = threadIdx.x; idx < a.nb << LOGM; idx += blockDim.x) {
-    int i = idx / a.nb, c = idx - i * a.nb;
-    sm[c * P + fft_phys(i)] = in[(size_t)i * a.n + c];
-  }
-  __syncthreads();
-  block_fft<LOGM, +1>(sm, a.nb, P, a.tw);
-  float2* out = a.out + (size_t)pl * a.n * a.n + c0;
-  for (int idx = threadIdx.x; idx < a.nb * a.n; idx += blockDim.x) {
-    int ix = idx / a.nb, c = idx - ix * a.nb, x = ix - a.n / 2;
-    float2 v = sm[c * P + fft_phys(fft_pos<LOGM>(x & (M - 1)))];
-    if (x & 1) { v.x = -v.x; v.y = -v.y; }
-    out[(size_t)ix * a.n + c] = v;
-  }
+  const int n = a.n, hn = a.n / 2;
+  const float2* in = a.in + (size_t)pl * M * n + c0;
+  float2* out = a.out + (size_t)pl * n * n + c0;
+  auto ld = [&](int t, int i) -> float2 { return in[(size_t)i * n + t]; };
+  auto st = [&](int t, int k, float2 v) {
+    int ix = k < hn ? k + hn : k - (M - hn);
+    if (k >= hn && k < M - hn) return;
+    if (k & 1) { v.x = -v.x; v.y = -v.y; }
+    out[(size_t)ix * n + t] = v;
+  };
+  block_fft<LOGM, +1, true, true>(sm, a.nb, a.lnb, P, a.tw, ld, st);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// x3 stage, one block per (x2, group of cb x1): xi3 = k_v cos(phi)/h depends on k_v only (Eq. 6), so the planes
+// x3 stage, one block per (x2, group of 8 x1): xi3 = k_v cos(phi)/h depends on k_v only (Eq. 6), so the planes
 // A[p] are samples of a 1-D unequally spaced spectrum along x3 for every (x1, x2):
 //   Gz[m3] = sum_p A[p] kap(t3(p) - m3),  t3 = M3 k_v cos(phi)/h;   vol[x3] = Re sum_m3 Gz[m3] e^{2 pi i x3 m3/M3}
 //   divided by kaphat(x1/M) kaphat(x2/M) kaphat(x3/M3)  (PAPER.md:136 step 1, reversed per PAPER.md:140).
+// The gridding is a banded matrix that is the same for every column: for grid cell i the planes with a tap on it
+// are contiguous, [zlo[i], zlo[i] + KZ), with weights ztab[i][KZ] (zero padded); the k_v = -h/2 plane (stored
+// last) has its own weight zlast[i].  Cell values are computed on the fly by the loader of the first FFT pass.
 // ---------------------------------------------------------------------------------------------------------------
+constexpr int kZCb = 8, kZLog = 3;
+
 struct ZArgs {
   const float2* A;       // [h/2+1][n][n]
   float* vol;            // output buffer; element (ix3, ix2, ix1) at vol[ix3*zstride + (ix2 - vol_x2_0)*n + ix1]
   size_t zstride;
   const float2* tw;      // length M3
-  const float* wz;       // [h/2+1][W] tap weights of plane p
-  const int* bz;         // [h/2+1] first tap m3 of plane p
-  const int2* prange;    // [M3] planes [lo, hi] (p < h/2 only) with a tap on stored index i (= m3 mod M3); lo > hi: none
+  const float* ztab;     // [M3][KZ]
+  const int* zlo;        // [M3]
+  const float* zlast;    // [M3]
   const float* dx;       // [n]  1/kaphat(x/M)
   const float* dz;       // [nz] 1/kaphat(x3/M3)
-  int n, nz, np, cb, W;
+  int n, nz, np, KZ;
   int x2_0;              // first x2 row of this launch
   int vol_x2_0;          // x2 index held by row 0 of the output buffer
 };
 
 template <int LOGM3>
 __global__ void __launch_bounds__(256) k_zstage(ZArgs a) {
-  constexpr int M3 = 1 << LOGM3, P = fft_pitch(M3);
+  constexpr int M3 = 1 << LOGM3, P = fft_tfast_pitch(M3, kZCb);
   extern __shared__ float2 sm[];
-  float2* Ain = sm;                       // [np][cb]
-  float2* Gz = sm + (size_t)a.np * a.cb;  // [cb][P]
-  const int ix2 = a.x2_0 + blockIdx.y, c0 = blockIdx.x * a.cb;
+  float2* Gz = sm;                                // [8][P]
+  float2* Ain = sm + kZCb * P;                    // [np + KZ][8], the KZ extra planes are zero
+  const int ix2 = a.x2_0 + blockIdx.y, c0 = blockIdx.x * kZCb;
   const size_t nn = (size_t)a.n * a.n;
   const float2* Ab = a.A + (size_t)ix2 * a.n + c0;
-  for (int idx = threadIdx.x; idx < a.np * a.cb; idx += blockDim.x) {
-    int p = idx / a.cb, c = idx - p * a.cb;
-    Ain[idx] = Ab[(size_t)p * nn + c];
+  for (int idx = threadIdx.x; idx < (a.np + a.KZ) * kZCb; idx += blockDim.x) {
+    int p = idx >> kZLog, c = idx & (kZCb - 1);
+    Ain[idx] = p < a.np ? Ab[(size_t)p * nn + c] : make_float2(0.f, 0.f);
   }
   __syncthreads();
-  for (int idx = threadIdx.x; idx < a.cb << LOGM3; idx += blockDim.x) {
-    int i = idx / a.cb, c = idx - i * a.cb;
-    int2 pr = a.prange[i];
-    float2 acc = make_float2(0.f, 0.f);
-    for (int p = pr.x; p <= pr.y; ++p) {
-      int j = (i - a.bz[p]) & (M3 - 1);
-      if (j < a.W) {
-        float wv = a.wz[p * a.W + j];
-        float2 v = Ain[p * a.cb + c];
-        acc.x = fmaf(v.x, wv, acc.x);
-        acc.y = fmaf(v.y, wv, acc.y);
-      }
+  const int KZ = a.KZ, last = (a.np - 1) * kZCb;
+  auto ld = [&](int t, int i) -> float2 {
+    const float* wt = a.ztab + (size_t)i * KZ;
+    const float2* ap = Ain + __ldg(&a.zlo[i]) * kZCb + t;
+    float wl = __ldg(&a.zlast[i]);
+    float2 v = Ain[last + t];
+    float2 acc = make_float2(v.x * wl, v.y * wl);
+    for (int s = 0; s < KZ; ++s) {
+      float wv = __ldg(&wt[s]);
+      float2 x = ap[s * kZCb];
+      acc.x = fmaf(x.x, wv, acc.x);
+      acc.y = fmaf(x.y, wv, acc.y);
     }
-    Gz[c * P + fft_phys(i)] = acc;
-  }
-  __syncthreads();
-  {  // the k_v = -h/2 plane (p = np-1) is out of order: scatter its W taps (one thread per (tap, column))
-    int p = a.np - 1;
-    for (int idx = threadIdx.x; idx < a.W * a.cb; idx += blockDim.x) {
-      int j = idx / a.cb, c = idx - j * a.cb;
-      int m = a.bz[p] + j, i = m & (M3 - 1);
-      float wv = a.wz[p * a.W + j];
-      float2 v = Ain[p * a.cb + c];
-      float2* g = &Gz[c * P + fft_phys(i)];
-      g->x = fmaf(v.x, wv, g->x);
-      g->y = fmaf(v.y, wv, g->y);
-    }
-  }
-  __syncthreads();
-  block_fft<LOGM3, +1>(Gz, a.cb, P, a.tw);
+    return acc;
+  };
   const float dx2 = a.dx[ix2];
+  const int hz = a.nz / 2;
   float* vb = a.vol + (size_t)(ix2 - a.vol_x2_0) * a.n + c0;
-  for (int idx = threadIdx.x; idx < a.nz * a.cb; idx += blockDim.x) {
-    int ix3 = idx / a.cb, c = idx - ix3 * a.cb, x3 = ix3 - a.nz / 2;
-    float v = Gz[c * P + fft_phys(fft_pos<LOGM3>(x3 & (M3 - 1)))].x;
-    vb[(size_t)ix3 * a.zstride + c] = v * a.dz[ix3] * dx2 * a.dx[c0 + c];
-  }
+  auto st = [&](int t, int k, float2 v) {
+    int ix3 = k < hz ? k + hz : k - (M3 - hz);
+    if (k >= hz && k < M3 - hz) return;
+    vb[(size_t)ix3 * a.zstride + t] = v.x * a.dz[ix3] * dx2 * a.dx[c0 + t];
+  };
+  block_fft<LOGM3, +1, true, true>(Gz, kZCb, kZLog, P, a.tw, ld, st);
 }
 
 }  // namespace lam
