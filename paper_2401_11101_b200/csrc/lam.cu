@@ -365,11 +365,11 @@ lam_status make_tables(lam_plan* p) {
   g.rho_unit = (double)M * std::sin(p->phi) / h;
   g.a1 = (float)M / (float)w;
   g.M = M;
-  g.nt = M / kTile;
+  g.nt = (M + kTile - 1) / kTile;
   g.ntheta = p->ntheta;
   g.w = w;
   g.hh = h / 2;
-  g.kstride = std::max(1, (int)std::ceil(1.0002 * std::sqrt(2.0) * w / M));
+  g.kstride = std::max(1, (int)std::ceil(1.0002 * std::sqrt(2.0) * W * w / M));  // samples between concurrently spread slots
   return LAM_OK;
 }
 
@@ -437,7 +437,7 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   const int lo = 1 << kLogMin, hi = 1 << kLogMax;
   if (w < lo || w > hi || h < lo || h > hi || M < 64 || M > hi || M3 < lo || M3 > hi)
     return fail(nullptr, LAM_EUNSUPPORTED, "w, h, sigma*nz must be in [32, 8192] and sigma*n in [64, 8192]");
-  if (h / 2 + 1 > 0x1fff || M / kTile > 0x1ff || n_theta > 0x3fff)
+  if (h / 2 + 1 > 0x1fff || (M + kTile - 1) / kTile > 0x1ff || n_theta > 0x3fff)
     return fail(nullptr, LAM_EUNSUPPORTED, "h <= 16382, sigma*n <= 16352 and n_theta <= 16383 in this build");
   if (M3 < 2 * P.width || M < 2 * P.width) return fail(nullptr, LAM_EINVAL, "grid smaller than the kernel footprint");
 
@@ -478,10 +478,10 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   if (cudaMemGetInfo(&freeb, &totalb) != cudaSuccess) return bail(fail(p, LAM_ECUDA, "cudaMemGetInfo failed"));
   size_t budget = P.device_bytes ? P.device_bytes : (size_t)(0.9 * (double)freeb);
   const size_t gplane = (size_t)M * M * 8, tplane = (size_t)M * n * 8;
-  p->PB = P.plane_batch > 0 ? P.plane_batch : (int)std::max<size_t>(1, std::min<size_t>(p->NP, (96u << 20) / (gplane + tplane)));
+  p->PB = P.plane_batch > 0 ? P.plane_batch : (int)std::max<size_t>(1, std::min<size_t>(p->NP, ((size_t)1 << 30) / (gplane + tplane)));
   p->PB = std::min(p->PB, p->NP);
   const size_t rproj = (size_t)h * p->WR * 8;
-  p->TC = P.theta_chunk > 0 ? P.theta_chunk : (int)std::max<size_t>(1, std::min<size_t>(n_theta, (32u << 20) / rproj));
+  p->TC = P.theta_chunk > 0 ? P.theta_chunk : (int)std::max<size_t>(1, std::min<size_t>(n_theta, ((size_t)256 << 20) / rproj));
   p->TC = std::min(p->TC, n_theta);
   const size_t need = (size_t)p->TC * rproj + (size_t)p->NP * n_theta * p->WQ * 8 + (size_t)p->PB * (gplane + tplane) +
                       (size_t)p->NP * n * n * 8 + p->device_bytes;
@@ -549,13 +549,12 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
   SpreadArgs sa{p->geom, p->kp, p->d_jobs + p->job_off[p0], p->job_off[p0 + np] - p->job_off[p0], p->d_S, p->WQ, p->d_G, p0};
   {
     StageScope sc(p, 1, s);
-    unsigned blocks = (unsigned)((sa.njobs + kSpreadWarps - 1) / kSpreadWarps);
-    k_zero_tiles<<<blocks, kSpreadWarps * 32, 0, s>>>(sa);
-    size_t sm = (size_t)kSpreadWarps * kTile * kTilePitch * sizeof(float2);
+    k_zero_tiles<<<(unsigned)((sa.njobs + 7) / 8), 256, 0, s>>>(sa);
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;
+      size_t sm = ((size_t)(kTile + 2 * W - 2) * kTP + 2 * kStage) * sizeof(float2);
       cudaFuncSetAttribute(k_spread<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-      k_spread<W><<<blocks, kSpreadWarps * 32, sm, s>>>(sa);
+      k_spread<W><<<(unsigned)sa.njobs, 32, sm, s>>>(sa);
     });
   }
   {

@@ -18,9 +18,15 @@
 
 namespace lam {
 
-constexpr int kTile = 32;               // gridding tile edge (fine-grid cells)
-constexpr int kTilePitch = kTile + 1;   // float2 elements per tile row in shared memory
-constexpr int kSpreadWarps = 8;         // warps (= private tiles) per k_spread block
+#ifndef LAM_TILE
+#define LAM_TILE 32
+#define LAM_TP 48
+#define LAM_NU 1
+#endif
+constexpr int kTile = LAM_TILE;               // gridding tile edge (fine-grid cells owned by a job)
+constexpr int kTP = LAM_TP;                 // float2 elements per storage row in shared memory (multiple of 16, >= kTile + 2W - 2)
+constexpr int kNU = LAM_NU;                  // samples a lane spreads per step (4*kNU concurrent slots per warp)
+constexpr int kStage = 64;              // samples of one line segment parked in shared memory
 constexpr int kJobSegs = 32;            // target segments (theta crossings) per job
 constexpr int kJobMaxSpan = 1023;       // max theta span of one job (10 bits)
 constexpr int kMaxW = 8;
@@ -141,12 +147,13 @@ struct KerPoly {
   float O[kMaxW / 2][kPolyHalf];
 };
 
-// job word layout: x = tx[0:9) ty[9:18) th0[18:32);  y = nth[0:10) mx[10:13) my[13:16) flags[16:18) p[18:31)
+// job word layout: x = tx[0:9) ty[9:18) th0[18:32);  y = nth[0:10) mx[10:13) my[13:16) flags[16:18) p[18:31) ydom[31]
 constexpr unsigned kJobExclusive = 1u, kJobFirstMulti = 2u;
 
-__device__ __forceinline__ uint2 job_pack(int tx, int ty, int th0, int nth, int mx, int my, unsigned fl, int p) {
+__device__ __forceinline__ uint2 job_pack(int tx, int ty, int th0, int nth, int mx, int my, unsigned fl, int p, int ydom) {
   return make_uint2((unsigned)tx | ((unsigned)ty << 9) | ((unsigned)th0 << 18),
-                    (unsigned)nth | ((unsigned)mx << 10) | ((unsigned)my << 13) | (fl << 16) | ((unsigned)p << 18));
+                    (unsigned)nth | ((unsigned)mx << 10) | ((unsigned)my << 13) | (fl << 16) | ((unsigned)p << 18) |
+                        ((unsigned)ydom << 31));
 }
 
 // ku range [ka, kb] of the samples of one line whose kernel footprint can reach the tile.
@@ -226,15 +233,15 @@ __global__ void k_jobs(JobsArgs a) {
       }
     }
   }
-  // pass B: emit jobs
+  // pass B: emit jobs; a job holds lines of one orientation only (|cos| >= |sin|: x-dominant, else y-dominant)
   unsigned njobs = 0;
-  int start = -1, last = -1, cnt = 0;
+  int start = -1, last = -1, cnt = 0, ori = 0;
   uint2* out = FILL ? a.jobs + a.off[gid] : nullptr;
   const unsigned total = FILL ? a.count[gid] : 0;
   auto emit = [&](int t0, int t1) {
     if (FILL) {
       unsigned fl = total == 1 ? kJobExclusive : (njobs == 0 ? kJobFirstMulti : 0u);
-      out[njobs] = job_pack(tx, ty, t0, t1 - t0, usex, usey, fl, p);
+      out[njobs] = job_pack(tx, ty, t0, t1 - t0, usex, usey, fl, p, ori);
     }
     ++njobs;
   };
@@ -242,6 +249,7 @@ __global__ void k_jobs(JobsArgs a) {
     for (int th = 0; th < g.ntheta; ++th) {
       double2 cs = g.cs[th];
       float c = (float)cs.x, s = (float)cs.y;
+      const int o = fabsf(c) >= fabsf(s) ? 0 : 1;
       bool hit = false;
       for (int sy = -1; sy <= 1 && !hit; ++sy) {
         if (!(usey >> (sy + 1) & 1)) continue;
@@ -254,20 +262,21 @@ __global__ void k_jobs(JobsArgs a) {
           hit = ka <= kb;
         }
       }
-      if (hit) {
-        if (start < 0) start = th;
-        ++cnt;
-        last = th;
-        if (cnt == kJobSegs || th + 1 - start >= kJobMaxSpan) { emit(start, th + 1); start = -1; cnt = 0; }
-      } else if (start >= 0 && th - last > 32) {
+      if (start >= 0 && (o != ori || (!hit && th - last > 32))) {
         emit(start, last + 1);
         start = -1;
         cnt = 0;
       }
+      if (hit) {
+        if (start < 0) { start = th; ori = o; }
+        ++cnt;
+        last = th;
+        if (cnt == kJobSegs || th + 1 - start >= kJobMaxSpan) { emit(start, th + 1); start = -1; cnt = 0; }
+      }
     }
     if (start >= 0) emit(start, last + 1);
   }
-  if (njobs == 0) emit(0, 0);  // untouched tile: one exclusive job that stores zeros
+  if (njobs == 0) { ori = 0; emit(0, 0); }  // untouched tile: one exclusive job that stores zeros
   if (!FILL) a.count[gid] = njobs;
 }
 
@@ -296,6 +305,23 @@ __device__ __forceinline__ void kernel_weights(const KerPoly& kp, float d, float
   }
 }
 
+template <int W>
+__device__ __forceinline__ void kernel_weights_r(const float (&E)[W / 2][kPolyHalf], const float (&O)[W / 2][kPolyHalf], float d,
+                                                 float (&wt)[W]) {
+  float d2 = d * d;
+#pragma unroll
+  for (int j = 0; j < W / 2; ++j) {
+    float e = E[j][3], o = O[j][3];
+#pragma unroll
+    for (int q = 2; q >= 0; --q) {
+      e = fmaf(e, d2, E[j][q]);
+      o = fmaf(o, d2, O[j][q]);
+    }
+    wt[j] = fmaf(d, o, e);
+    wt[W - 1 - j] = fmaf(-d, o, e);
+  }
+}
+
 struct SpreadArgs {
   SpreadGeom g;
   KerPoly kp;
@@ -307,38 +333,71 @@ struct SpreadArgs {
   int p0;              // first plane of the batch
 };
 
-// zero the tiles that receive atomic adds from several jobs
+// zero the tiles that receive atomic adds from several jobs (one warp per job word; only the first job of a tile acts)
 __global__ void k_zero_tiles(SpreadArgs a) {
   const int lane = threadIdx.x & 31;
   long long j = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (j >= a.njobs) return;
   uint2 jb = a.jobs[j];
   if (!((jb.y >> 16) & kJobFirstMulti)) return;
+  const int M = a.g.M;
   int tx = jb.x & 0x1ff, ty = (jb.x >> 9) & 0x1ff, p = (jb.y >> 18) & 0x1fff;
-  float2* Gp = a.G + (size_t)(p - a.p0) * a.g.M * a.g.M + (size_t)(ty * kTile) * a.g.M + tx * kTile;
-  for (int r = 0; r < kTile; ++r) Gp[(size_t)r * a.g.M + lane] = make_float2(0.f, 0.f);
+  float2* Gp = a.G + (size_t)(p - a.p0) * M * M;
+  const int x0 = tx * kTile, y0 = ty * kTile;
+  for (int r = 0; r < kTile && y0 + r < M; ++r)
+    for (int c = lane; c < kTile && x0 + c < M; c += 32) Gp[(size_t)(y0 + r) * M + x0 + c] = make_float2(0.f, 0.f);
 }
 
+// Spreading of one job.  The warp owns a private storage tile [kTile + 2W - 2][kTP] in shared memory that covers the
+// owned cells plus the kernel halo, so every tap of every visited sample lands inside it and needs no bounds test;
+// a sample is visited iff its W x W footprint meets the owned kTile x kTile cells.
+//
+// Lane roles: half-warp h holds two slots of W lanes; lane j of a slot owns tap column j of the slot's current
+// sample (along the MAJOR axis: x for x-dominant lines, y for y-dominant lines, whose jobs work on the transposed
+// tile) and walks the W taps of the minor axis.  The four slots take samples q apart on the same line,
+// q = ceil(W / sqrt 2): their footprints are disjoint (no lost update inside one instruction), and for W = 6 the
+// two runs of 6 contiguous cells of a half-warp sit 7..10 columns apart in rows whose pitch is a multiple of 16:
+// 12 distinct banks per 128-byte wavefront, no conflicts by construction.
 template <int W>
-__global__ void __launch_bounds__(kSpreadWarps * 32) k_spread(SpreadArgs a) {
-  extern __shared__ float2 sm[];
+__global__ void __launch_bounds__(32) k_spread(SpreadArgs a) {
+  extern __shared__ float2 tile[];
+  constexpr int H = W - 1;                           // low-side halo of the storage
+  constexpr int ROWS = kTile + 2 * W - 2;
   const SpreadGeom& g = a.g;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const long long jid = (long long)blockIdx.x * kSpreadWarps + warp;
-  if (jid >= a.njobs) return;  // no block-level barrier is used below
-  float2* tile = sm + warp * (kTile * kTilePitch);
+  const int Q = g.kstride;  // sample distance between slots (footprints disjoint)
+  const int lane = threadIdx.x;
+  const long long jid = blockIdx.x;
   const unsigned tile_addr = (unsigned)__cvta_generic_to_shared(tile);
   const uint2 jb = a.jobs[jid];
   const int tx = jb.x & 0x1ff, ty = (jb.x >> 9) & 0x1ff, th0 = jb.x >> 18;
   const int nth = jb.y & 0x3ff, usex = (jb.y >> 10) & 7, usey = (jb.y >> 13) & 7;
   const unsigned flags = (jb.y >> 16) & 3u;
   const int p = (jb.y >> 18) & 0x1fff;
+  const bool ydom = (jb.y >> 31) != 0;
   const int kv = p == g.hh ? -g.hh : p;
   const double rho = g.rho_unit * kv;
   const int mx0 = tx * kTile - g.M / 2, my0 = ty * kTile - g.M / 2;
   const int hw = g.w / 2;
 
-  for (int i = lane; i < kTile * kTilePitch; i += 32) tile[i] = make_float2(0.f, 0.f);
+  // lane role
+  const int hl = lane & 15, slot2 = hl / W, j1 = hl - slot2 * W;
+  const bool role = slot2 < 2;
+  const int sidx = 2 * (lane >> 4) + slot2;
+  const int slot_lane0 = role ? lane - j1 : lane;  // first lane of this lane's slot
+  float cE[kPolyHalf], cO[kPolyHalf];  // this lane's major-axis tap polynomial: E(d^2) + d O(d^2)
+  {
+    const int jj = role ? min(j1, W - 1 - j1) : 0;
+    const float sg = j1 < W / 2 ? 1.f : -1.f;
+#pragma unroll
+    for (int q = 0; q < kPolyHalf; ++q) {
+      cE[q] = a.kp.E[jj][q];
+      cO[q] = sg * a.kp.O[jj][q];
+    }
+  }
+
+  for (int i = lane; i < ROWS * kTP; i += 32) tile[i] = make_float2(0.f, 0.f);
+  float2* stg = tile + ROWS * kTP;  // [2][kStage] samples of the current / next line
+  int sb = 0;
   __syncwarp();
 
   const float2* Sp = a.S + (size_t)p * g.ntheta * a.WQ;
@@ -358,94 +417,141 @@ __global__ void __launch_bounds__(kSpreadWarps * 32) k_spread(SpreadArgs a) {
         // position of sample ka relative to the tile, in double (large terms cancel), then fp32
         const double u0 = (double)g.a1 * ka;
         const float p0x = (float)(oxd + u0 * cs.x), p0y = (float)(oyd + u0 * cs.y);
+        // major / minor axes of this job
+        const float lM0 = ydom ? p0y : p0x, lm0 = ydom ? p0x : p0y, lcM = ydom ? s : c, lcm = ydom ? c : s;
         unsigned mask = __ballot_sync(0xffffffffu, ka <= kb);
-        while (mask) {
-          const int src = __ffs(mask) - 1;
+        if (!mask) continue;
+        // lines of this batch, one after the other; the samples of the NEXT line are fetched into registers while
+        // the current line is spread, then parked in the staging buffer (double-buffered)
+        int src = __ffs(mask) - 1;
+        int ska = __shfl_sync(0xffffffffu, ka, src), n = __shfl_sync(0xffffffffu, kb, src) - ska + 1;
+        const float2* Srow = Sp + (size_t)(tb + src) * a.WQ + hw + ska;
+        stg[sb * kStage + lane] = lane < n ? __ldg(&Srow[lane]) : make_float2(0.f, 0.f);
+        stg[sb * kStage + lane + 32] = lane + 32 < n ? __ldg(&Srow[lane + 32]) : make_float2(0.f, 0.f);
+        while (true) {
+          const float aM = g.a1 * __shfl_sync(0xffffffffu, lcM, src), am = g.a1 * __shfl_sync(0xffffffffu, lcm, src);
+          const float M0 = __shfl_sync(0xffffffffu, lM0, src), m0 = __shfl_sync(0xffffffffu, lm0, src);
           mask &= mask - 1;
-          const int ska = __shfl_sync(0xffffffffu, ka, src), skb = __shfl_sync(0xffffffffu, kb, src);
-          const float sc = __shfl_sync(0xffffffffu, c, src), ss = __shfl_sync(0xffffffffu, s, src);
-          const float sx0 = __shfl_sync(0xffffffffu, p0x, src), sy0 = __shfl_sync(0xffffffffu, p0y, src);
-          const float2* Srow = Sp + (size_t)(tb + src) * a.WQ + hw;
-          const bool xdom = fabsf(sc) >= fabsf(ss);
-          // lanes take samples ska + sub + kstride*i so that two lanes never share a tap cell in one instruction
-          for (int sub = 0; sub < g.kstride; ++sub) {
-            for (int kbase = ska + sub; kbase <= skb; kbase += 32 * g.kstride) {
-              const int ku = kbase + lane * g.kstride;
-              const bool act = ku <= skb;
-              float2 v = act ? __ldg(&Srow[ku]) : make_float2(0.f, 0.f);
-              const float du = g.a1 * (float)(ku - ska);
-              const float t1 = fmaf(du, sc, sx0), t2 = fmaf(du, ss, sy0);
-              const float c1 = ceilf(t1 - 0.5f * W), c2 = ceilf(t2 - 0.5f * W);
-              const int col0 = (int)c1, row0 = (int)c2;
-              float w1[W], w2[W];
-              kernel_weights<W>(a.kp, t1 - c1 - (0.5f * W - 0.5f), w1);
-              kernel_weights<W>(a.kp, t2 - c2 - (0.5f * W - 0.5f), w2);
-              if (xdom) {
+          const bool more = mask != 0;
+          int nsrc = 0, nska = 0, nn = 0;
+          const float2* nSrow = Srow;
+          float2 nv0 = make_float2(0.f, 0.f), nv1 = nv0;
+          if (more) {
+            nsrc = __ffs(mask) - 1;
+            nska = __shfl_sync(0xffffffffu, ka, nsrc);
+            nn = __shfl_sync(0xffffffffu, kb, nsrc) - nska + 1;
+            nSrow = Sp + (size_t)(tb + nsrc) * a.WQ + hw + nska;
+            if (lane < nn) nv0 = __ldg(&nSrow[lane]);
+            if (lane + 32 < nn) nv1 = __ldg(&nSrow[lane + 32]);
+          }
+          __syncwarp();
+          for (int seg = 0; seg < n; seg += kStage) {
+            if (seg > 0) {  // long lines (small a1): later segments are fetched in place
+              __syncwarp();
+              stg[sb * kStage + lane] = seg + lane < n ? __ldg(&Srow[seg + lane]) : make_float2(0.f, 0.f);
+              stg[sb * kStage + lane + 32] = seg + lane + 32 < n ? __ldg(&Srow[seg + lane + 32]) : make_float2(0.f, 0.f);
+              __syncwarp();
+            }
+            const int nseg = min(n - seg, kStage);
+            // 4*kNU slots (kNU per lane) take samples Qe apart; one sweep of Qe steps covers the segment
+            const int Qe = max(Q, (nseg + 4 * kNU - 1) / (4 * kNU));
+#pragma unroll 1
+            for (int it = 0; it < Qe; ++it) {
+              float2 acc[kNU][W];
+              float wm[kNU][W];
+              float2 vw[kNU];
+              unsigned ad[kNU];
+              bool ok[kNU];
 #pragma unroll
-                for (int j1 = 0; j1 < W; ++j1) {
-                  const int col = col0 + j1;
-                  const bool okc = act && (unsigned)col < (unsigned)kTile;
-                  const float2 vw = make_float2(v.x * w1[j1], v.y * w1[j1]);
-                  float2 acc[W];
-                  bool ok[W];
-                  unsigned ad[W];
+              for (int u = 0; u < kNU; ++u) {
+                const int kk = (sidx + 4 * u) * Qe + it;
+                const float fk = (float)(seg + kk);
+                const float tM = fmaf(fk, aM, M0), tm = fmaf(fk, am, m0);
+                const float cf = ceilf(tM - 0.5f * W), rf = ceilf(tm - 0.5f * W);
+                const int col0 = (int)cf, row0 = (int)rf;
+                ok[u] = role && kk < nseg && (unsigned)(col0 + H) < (unsigned)(kTile + H) &&
+                        (unsigned)(row0 + H) < (unsigned)(kTile + H);
+                const float2 v = stg[sb * kStage + (kk & (kStage - 1))];
+                // this lane's tap polynomial at both offsets: its own major-axis weight, and minor-axis weight j1
+                // of the slot's sample, which the W lanes of the slot then exchange
+                const float dM = tM - cf - (0.5f * W - 0.5f), dm = tm - rf - (0.5f * W - 0.5f);
+                const float dM2 = dM * dM, dm2 = dm * dm;
+                float eM = cE[3], oM = cO[3], em = cE[3], om = cO[3];
 #pragma unroll
-                  for (int j2 = 0; j2 < W; ++j2) {
-                    const int row = row0 + j2;
-                    ok[j2] = okc && (unsigned)row < (unsigned)kTile;
-                    ad[j2] = tile_addr + (unsigned)(row * kTilePitch + col) * 8u;
-                    if (ok[j2]) acc[j2] = lds_v(ad[j2]);
-                  }
-#pragma unroll
-                  for (int j2 = 0; j2 < W; ++j2) {
-                    acc[j2].x = fmaf(vw.x, w2[j2], acc[j2].x);
-                    acc[j2].y = fmaf(vw.y, w2[j2], acc[j2].y);
-                  }
-#pragma unroll
-                  for (int j2 = 0; j2 < W; ++j2)
-                    if (ok[j2]) sts_v(ad[j2], acc[j2]);
+                for (int q = 2; q >= 0; --q) {
+                  eM = fmaf(eM, dM2, cE[q]);
+                  oM = fmaf(oM, dM2, cO[q]);
+                  em = fmaf(em, dm2, cE[q]);
+                  om = fmaf(om, dm2, cO[q]);
                 }
-              } else {
+                const float wM = fmaf(dM, oM, eM), wmine = fmaf(dm, om, em);
+#pragma unroll
+                for (int j2 = 0; j2 < W; ++j2) wm[u][j2] = __shfl_sync(0xffffffffu, wmine, slot_lane0 + j2);
+                vw[u] = make_float2(v.x * wM, v.y * wM);
+                ad[u] = tile_addr + (unsigned)((row0 + H) * kTP + col0 + H + j1) * 8u;
+              }
+#pragma unroll
+              for (int u = 0; u < kNU; ++u)
+#pragma unroll
+                for (int j2 = 0; j2 < W; ++j2)
+                  if (ok[u]) acc[u][j2] = lds_v(ad[u] + j2 * (kTP * 8));
+#pragma unroll
+              for (int u = 0; u < kNU; ++u)
 #pragma unroll
                 for (int j2 = 0; j2 < W; ++j2) {
-                  const int row = row0 + j2;
-                  const bool okr = act && (unsigned)row < (unsigned)kTile;
-                  const float2 vw = make_float2(v.x * w2[j2], v.y * w2[j2]);
-                  float2 acc[W];
-                  bool ok[W];
-                  unsigned ad[W];
-#pragma unroll
-                  for (int j1 = 0; j1 < W; ++j1) {
-                    const int col = col0 + j1;
-                    ok[j1] = okr && (unsigned)col < (unsigned)kTile;
-                    ad[j1] = tile_addr + (unsigned)(row * kTilePitch + col) * 8u;
-                    if (ok[j1]) acc[j1] = lds_v(ad[j1]);
-                  }
-#pragma unroll
-                  for (int j1 = 0; j1 < W; ++j1) {
-                    acc[j1].x = fmaf(vw.x, w1[j1], acc[j1].x);
-                    acc[j1].y = fmaf(vw.y, w1[j1], acc[j1].y);
-                  }
-#pragma unroll
-                  for (int j1 = 0; j1 < W; ++j1)
-                    if (ok[j1]) sts_v(ad[j1], acc[j1]);
+                  acc[u][j2].x = fmaf(vw[u].x, wm[u][j2], acc[u][j2].x);
+                  acc[u][j2].y = fmaf(vw[u].y, wm[u][j2], acc[u][j2].y);
                 }
-              }
+#pragma unroll
+              for (int u = 0; u < kNU; ++u)
+#pragma unroll
+                for (int j2 = 0; j2 < W; ++j2)
+                  if (ok[u]) sts_v(ad[u] + j2 * (kTP * 8), acc[u][j2]);
             }
           }
+          if (!more) break;
+          sb ^= 1;
+          stg[sb * kStage + lane] = nv0;
+          stg[sb * kStage + lane + 32] = nv1;
+          src = nsrc;
+          ska = nska;
+          n = nn;
+          Srow = nSrow;
         }
+        __syncwarp();
       }
     }
   }
   __syncwarp();
-  float2* Gp = a.G + (size_t)(p - a.p0) * g.M * g.M + (size_t)(ty * kTile) * g.M + tx * kTile;
-  if (flags & kJobExclusive) {
-    for (int r = 0; r < kTile; ++r) Gp[(size_t)r * g.M + lane] = lds_v(tile_addr + (unsigned)(r * kTilePitch + lane) * 8u);
-  } else {
-    for (int r = 0; r < kTile; ++r) {
-      float2 v = lds_v(tile_addr + (unsigned)(r * kTilePitch + lane) * 8u);
-      if (v.x != 0.f || v.y != 0.f) atomicAdd(&Gp[(size_t)r * g.M + lane], v);
+  // y-dominant jobs worked on the transposed tile: transpose the owned square in place (diagonal sweeps: lane i swaps
+  // (i, i+r) with (i+r, i); both accesses of an instruction touch distinct banks)
+  if (ydom) {
+    for (int r = 1; r <= kTile / 2; ++r) {
+      for (int i = lane; i < kTile; i += 32) {
+        if (2 * r == kTile && i >= kTile / 2) continue;
+        int j = i + r;
+        if (j >= kTile) j -= kTile;
+        const unsigned a1 = tile_addr + (unsigned)((i + H) * kTP + j + H) * 8u;
+        const unsigned a2 = tile_addr + (unsigned)((j + H) * kTP + i + H) * 8u;
+        float2 u = lds_v(a1), v = lds_v(a2);
+        sts_v(a1, v);
+        sts_v(a2, u);
+      }
     }
+    __syncwarp();
+  }
+  const int M = g.M, x0 = tx * kTile, y0 = ty * kTile;
+  float2* Gp = a.G + (size_t)(p - a.p0) * M * M;
+  if (flags & kJobExclusive) {
+    for (int r = 0; r < kTile && y0 + r < M; ++r)
+      for (int cc = lane; cc < kTile && x0 + cc < M; cc += 32)
+        Gp[(size_t)(y0 + r) * M + x0 + cc] = lds_v(tile_addr + (unsigned)((r + H) * kTP + cc + H) * 8u);
+  } else {
+    for (int r = 0; r < kTile && y0 + r < M; ++r)
+      for (int cc = lane; cc < kTile && x0 + cc < M; cc += 32) {
+        float2 v = lds_v(tile_addr + (unsigned)((r + H) * kTP + cc + H) * 8u);
+        if (v.x != 0.f || v.y != 0.f) atomicAdd(&Gp[(size_t)(y0 + r) * M + x0 + cc], v);
+      }
   }
 }
 

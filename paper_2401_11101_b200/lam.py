@@ -13,7 +13,7 @@ import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
-LIB_PATH = os.path.join(_HERE, "liblam.so")
+LIB_PATH = os.environ.get("LAM_LIB") or os.path.join(_HERE, "liblam.so")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 
 LAM_OK, LAM_EINVAL, LAM_ENOMEM_DEVICE, LAM_ENOMEM_HOST, LAM_ECUDA, LAM_EUNSUPPORTED = range(6)
