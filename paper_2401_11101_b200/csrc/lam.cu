@@ -24,6 +24,11 @@ using namespace lam;
 namespace {
 
 thread_local std::string g_create_error;
+thread_local cudaError_t g_launch_error = cudaSuccess;  // first failed kernel launch of the current call
+inline void note_launch() {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess && g_launch_error == cudaSuccess) g_launch_error = e;
+}
 
 struct StageEvent {
   int stage;
@@ -55,7 +60,8 @@ struct lam_plan {
   uint2* d_jobs = nullptr;
   std::vector<long long> job_off;  // [NP+1] first job of each plane
   // workspace
-  float2 *d_R = nullptr, *d_S = nullptr, *d_G = nullptr, *d_T = nullptr, *d_A = nullptr;
+  float2 *d_R = nullptr, *d_S = nullptr, *d_G = nullptr, *d_T = nullptr, *d_A = nullptr;  // d_S, d_A live inside d_arena
+  float2* d_arena = nullptr;
   size_t device_bytes = 0, pinned_bytes = 0;
   bool have_darkflat = false;
   // host-pointer path (allocated on first use): device staging, copy streams, hand-over events
@@ -143,26 +149,32 @@ struct Launch {
     if (raw) {
       cudaFuncSetAttribute(k_rows<L, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
       k_rows<L, true><<<g, 256, sm, s>>>(a);
+      note_launch();
     } else {
       cudaFuncSetAttribute(k_rows<L, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
       k_rows<L, false><<<g, 256, sm, s>>>(a);
+      note_launch();
     }
   }
   static void cols(dim3 g, int threads, size_t sm, cudaStream_t s, const ColsArgs& a) {
     cudaFuncSetAttribute(k_cols<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     k_cols<L><<<g, threads, sm, s>>>(a);
+      note_launch();
   }
   static void x1(dim3 g, size_t sm, cudaStream_t s, const IfftArgs& a) {
     cudaFuncSetAttribute(k_ifft_x1<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     k_ifft_x1<L><<<g, 256, sm, s>>>(a);
+      note_launch();
   }
   static void x2(dim3 g, int threads, size_t sm, cudaStream_t s, const IfftArgs& a) {
     cudaFuncSetAttribute(k_ifft_x2<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     k_ifft_x2<L><<<g, threads, sm, s>>>(a);
+      note_launch();
   }
   static void z(dim3 g, size_t sm, cudaStream_t s, const ZArgs& a) {
     cudaFuncSetAttribute(k_zstage<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     k_zstage<L><<<g, 256, sm, s>>>(a);
+      note_launch();
   }
 };
 
@@ -207,7 +219,7 @@ struct StageScope {
 void free_all(lam_plan* p) {
   void* ptrs[] = {p->d_cs,    p->d_Pu,  p->d_Pv,  p->d_PuNone, p->d_tw_w, p->d_tw_h,   p->d_tw_M, p->d_tw_M3,
                   p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs,
-                  p->d_R,     p->d_S,   p->d_G,   p->d_T,      p->d_A};
+                  p->d_R,     p->d_arena, p->d_G, p->d_T};
   for (void* q : ptrs)
     if (q) cudaFree(q);
   for (int i = 0; i < 2; ++i) {
@@ -483,18 +495,20 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   const size_t rproj = (size_t)h * p->WR * 8;
   p->TC = P.theta_chunk > 0 ? P.theta_chunk : (int)std::max<size_t>(1, std::min<size_t>(n_theta, ((size_t)256 << 20) / rproj));
   p->TC = std::min(p->TC, n_theta);
-  const size_t need = (size_t)p->TC * rproj + (size_t)p->NP * n_theta * p->WQ * 8 + (size_t)p->PB * (gplane + tplane) +
-                      (size_t)p->NP * n * n * 8 + p->device_bytes;
+  // The spectra planes S[p] die as the planes are gridded and the cropped planes A[p] are born at the same pace, so both
+  // share one arena: A grows from the front, S sits right-aligned at the back; a batch of PB planes may be in flight.
+  const size_t splane = (size_t)n_theta * p->WQ, aplane = (size_t)n * n;
+  const size_t arena = std::max((size_t)p->PB * aplane + (size_t)p->NP * splane, (size_t)p->NP * aplane + (size_t)p->PB * splane);
+  const size_t need = (size_t)p->TC * rproj + arena * 8 + (size_t)p->PB * (gplane + tplane) + p->device_bytes;
   if (need > budget)
     return bail(fail(p, LAM_ENOMEM_DEVICE, "in-core workspace of %.2f GB exceeds the budget of %.2f GB", need / 1e9, budget / 1e9));
   if ((st = dalloc(p, &p->d_R, (size_t)p->TC * h * p->WR)) != LAM_OK) return bail(st);
-  if ((st = dalloc(p, &p->d_S, (size_t)p->NP * n_theta * p->WQ)) != LAM_OK) return bail(st);
+  if ((st = dalloc(p, &p->d_arena, arena)) != LAM_OK) return bail(st);
+  p->d_A = p->d_arena;
+  p->d_S = p->d_arena + (arena - (size_t)p->NP * splane);
   if ((st = dalloc(p, &p->d_G, (size_t)p->PB * M * M)) != LAM_OK) return bail(st);
   if ((st = dalloc(p, &p->d_T, (size_t)p->PB * M * n)) != LAM_OK) return bail(st);
-  if ((st = dalloc(p, &p->d_A, (size_t)p->NP * n * n)) != LAM_OK) return bail(st);
   if ((st = build_jobs(p)) != LAM_OK) return bail(st);
-  // the q = w slot and the row padding of S are read by k_spread: keep them defined
-  if (cudaMemset(p->d_S, 0, (size_t)p->NP * n_theta * p->WQ * 8) != cudaSuccess) return bail(fail(p, LAM_ECUDA, "memset failed"));
   if (cudaDeviceSynchronize() != cudaSuccess) return bail(fail(p, LAM_ECUDA, "plan setup failed: %s", cudaGetErrorString(cudaGetLastError())));
   *out = p;
   return LAM_OK;
@@ -550,11 +564,13 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
   {
     StageScope sc(p, 1, s);
     k_zero_tiles<<<(unsigned)((sa.njobs + 7) / 8), 256, 0, s>>>(sa);
+      note_launch();
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;
       size_t sm = ((size_t)(kTile + 2 * W - 2) * kTP + 2 * kStage) * sizeof(float2);
       cudaFuncSetAttribute(k_spread<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
       k_spread<W><<<(unsigned)sa.njobs, 32, sm, s>>>(sa);
+      note_launch();
     });
   }
   {
@@ -613,6 +629,7 @@ lam_status lam_backproject(lam_plan* p, const void* proj, float* vol, void* cuda
     if (st != LAM_OK) return st;
   }
   p->launches = 0;
+  g_launch_error = cudaSuccess;
   p->events_used = 0;
   p->stage_valid = false;
   const size_t esz = p->prm.input == LAM_INPUT_U16_RAW ? 2 : 4;
@@ -670,6 +687,7 @@ lam_status lam_backproject(lam_plan* p, const void* proj, float* vol, void* cuda
     }
   }
   CU(p, cudaGetLastError());
+  if (g_launch_error != cudaSuccess) return fail(p, LAM_ECUDA, "kernel launch failed: %s", cudaGetErrorString(g_launch_error));
   p->stage_valid = p->profiling;
   if (!vol_dev) CU(p, cudaStreamSynchronize(p->s_d2h));  // host results are valid on return
   return LAM_OK;

@@ -94,7 +94,7 @@ struct ColsArgs {
 
 
 template <int LOGH>
-__global__ void __launch_bounds__(256) k_cols(ColsArgs a) {
+__global__ void __launch_bounds__(512) k_cols(ColsArgs a) {
   constexpr int h = 1 << LOGH;
   extern __shared__ float2 sm[];
   const int kColsLog = a.lcb, kColsCb = 1 << a.lcb, P = fft_tfast_pitch(h, kColsCb);

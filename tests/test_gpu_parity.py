@@ -163,3 +163,21 @@ def test_errors_do_not_cross_the_boundary():
     with pytest.raises(lam.LamError):                   # dark/flat missing
         plan.backproject(torch.zeros((2, 64, 64), dtype=torch.uint16, device="cuda"))
     plan.close()
+
+
+@pytest.mark.parametrize("n,nz,h,w,nth", [(2048, 32, 64, 64, 6),      # sigma*n = 4096: three radix-16 passes
+                                          (1024, 32, 2048, 64, 6),    # h = 2048: 512-thread column FFT
+                                          (256, 512, 64, 2048, 6),    # w = 2048, sigma*nz = 1024
+                                          (4096, 16, 32, 32, 4),      # sigma*n = 8192: four passes, 2 columns per block
+                                          (256, 16, 4096, 32, 4)])    # h = 4096: 4 columns per block
+def test_long_transform_lengths_against_exact_columns(n, nz, h, w, nth):
+    """Every FFT length / block shape the full-size configs use, on thin problems the exact oracle can follow."""
+    cfg = inputs.Config(f"fft{n}x{h}x{w}", n, nz, h, w, nth, 20.0, 12, min(nz / 4, h / 8), seed=5)
+    d = inputs.projections(cfg)
+    vol, _ = run_gpu(cfg, d)
+    rng = np.random.default_rng(1)
+    r = min(n // 4, w // 3)
+    cols = (n // 2 + rng.integers(-r, r, size=(6, 2))).astype(np.int32)
+    ref = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy(), cols=cols)
+    got = np.stack([vol[:, c[1], c[0]] for c in cols])
+    assert rel(got, ref) <= GATE_TINY
