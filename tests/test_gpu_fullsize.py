@@ -75,3 +75,29 @@ def test_full_size_sparse_angles_against_exact_columns(idx):
     del proj
     err = check_columns(cfg, vol, sel, proj_sel, dark, flat)
     print(f"configs[{idx}] full size: rel L2 on {NCOLS} exact columns = {err:.3e}, plan = {info}")
+
+
+def test_config4_out_of_core_host_buffers():
+    """configs[4]: 4096 x 4096 x 1024 volume (64 GiB) from 3000 uint16 projections of 2048 x 4096 (47 GiB), both in
+    pinned HOST memory; lam_backproject streams chunks in and slabs out on its copy streams."""
+    import psutil
+    cfg = inputs.config(4)
+    free, _ = torch.cuda.mem_get_info()
+    need_host = cfg.ntheta * cfg.h * cfg.w * 2 + cfg.voxels * 4
+    if free < 150e9 or psutil.virtual_memory().available < need_host + 20e9:
+        pytest.skip("configs[4] needs ~145 GB of device memory and ~135 GB of host memory")
+    proj, sel, proj_sel, dark, flat = sparse_scan(cfg, "cpu")
+    vol = torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, pin_memory=True)
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
+                    input="u16")
+    plan.set_darkflat(dark.cuda(), flat.cuda())
+    import time
+    t0 = time.perf_counter()
+    lam.lam_backproject(plan._plan, proj.data_ptr(), vol.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    info = plan.info()
+    plan.close()
+    err = check_columns(cfg, vol, sel, proj_sel, dark, flat)
+    print(f"configs[4] out-of-core: {dt:.2f} s wall ({cfg.voxels / dt / 1e9:.2f} GVoxel/s incl. PCIe), rel L2 on {NCOLS} "
+          f"exact columns = {err:.3e}, plan = {info}")
