@@ -155,13 +155,19 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfg = inputs.config(args.config)
-    d = inputs.projections(cfg, device="cuda")
+    hostmode = cfg.out_of_core  # configs[4]: input + workspace exceed HBM; projections and volume live in pinned host memory
+    if hostmode:
+        out = torch.empty((cfg.ntheta, cfg.h, cfg.w), dtype=torch.uint16 if cfg.raw16 else torch.float32, pin_memory=True)
+        d = inputs.projections(cfg, device="cuda", out=out)
+    else:
+        d = inputs.projections(cfg, device="cuda")
     proj = d["proj"]
     plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
                     input="u16" if cfg.raw16 else "f32")
     if cfg.raw16:
         plan.set_darkflat(d["dark"], d["flat"])
-    vol = torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, device="cuda")
+    vol = (torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, pin_memory=True) if hostmode else
+           torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, device="cuda"))
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -203,7 +209,7 @@ def run_ours(args):
 
     # ---- e2e: the same call with host (pinned) buffers; H2D + D2H inside the timed region
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not hostmode:
         hproj = torch.empty(proj.shape, dtype=proj.dtype, pin_memory=True)
         hproj.copy_(proj)
         hvol = torch.empty(vol.shape, dtype=torch.float32, pin_memory=True)
@@ -228,6 +234,10 @@ def run_ours(args):
                "h2d_bytes_per_step": hproj.numel() * hproj.element_size(),
                "d2h_bytes_per_step": hvol.numel() * 4, "host_vs_device_result_rel_l2": err}
         del hproj, hvol
+    if hostmode:  # the timed call above already ran host -> host
+        e2e = {"value": value, "unit": UNIT, "ms_per_step": ms_step, "steps": args.steps,
+               "h2d_bytes_per_step": proj.numel() * proj.element_size(), "d2h_bytes_per_step": vol.numel() * 4,
+               "note": "configs[4] does not fit HBM: value and e2e are the same host-buffer run"}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

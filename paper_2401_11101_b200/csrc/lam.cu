@@ -56,7 +56,7 @@ struct lam_plan {
   float2 *d_Pu = nullptr, *d_Pv = nullptr, *d_PuNone = nullptr;
   float2 *d_tw_w = nullptr, *d_tw_h = nullptr, *d_tw_M = nullptr, *d_tw_M3 = nullptr;
   float *d_ztab = nullptr, *d_zlast = nullptr, *d_dx = nullptr, *d_dz = nullptr, *d_dark = nullptr, *d_flat = nullptr;
-  int* d_zlo = nullptr;
+  int *d_zlo = nullptr, *d_zcnt = nullptr;
   uint2* d_jobs = nullptr;
   std::vector<long long> job_off;  // [NP+1] first job of each plane
   // workspace
@@ -218,7 +218,7 @@ struct StageScope {
 
 void free_all(lam_plan* p) {
   void* ptrs[] = {p->d_cs,    p->d_Pu,  p->d_Pv,  p->d_PuNone, p->d_tw_w, p->d_tw_h,   p->d_tw_M, p->d_tw_M3,
-                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs,
+                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_zcnt,
                   p->d_R,     p->d_arena, p->d_G, p->d_T};
   for (void* q : ptrs)
     if (q) cudaFree(q);
@@ -363,7 +363,10 @@ lam_status make_tables(lam_plan* p) {
       }
     }
     if ((st = upload(p, &p->d_ztab, ztab)) != LAM_OK) return st;
+    std::vector<int> cnt(M3);
+    for (int i = 0; i < M3; ++i) cnt[i] = hi[i] >= lo[i] ? hi[i] - lo[i] + 1 : 0;
     if ((st = upload(p, &p->d_zlo, lo)) != LAM_OK) return st;
+    if ((st = upload(p, &p->d_zcnt, cnt)) != LAM_OK) return st;
     if ((st = upload(p, &p->d_zlast, zlast)) != LAM_OK) return st;
   }
   std::vector<float> dx(n), dz(nz);
@@ -588,7 +591,7 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
 // x3 stage for x2 rows [x2_0, x2_0 + rows); out holds x2 row `out_x2_0` in its first row, z-stride `zstride` floats
 static void launch_z(lam_plan* p, float* out, size_t zstride, int x2_0, int rows, int out_x2_0, cudaStream_t s) {
   StageScope sc(p, 3, s);
-  ZArgs za{p->d_A, out, zstride, p->d_tw_M3, p->d_ztab, p->d_zlo, p->d_zlast, p->d_dx, p->d_dz,
+  ZArgs za{p->d_A, out, zstride, p->d_tw_M3, p->d_ztab, p->d_zlo, p->d_zcnt, p->d_zlast, p->d_dx, p->d_dz,
            p->n, p->nz, p->NP, p->KZ, x2_0, out_x2_0};
   DISPATCH_LOG(p->logM3, z(dim3(p->n / kZCb, rows), zstage_smem(p), s, za));
   p->launches += 1;

@@ -23,6 +23,9 @@ namespace lam {
 #define LAM_TP 48
 #define LAM_NU 1
 #endif
+#ifndef LAM_QL
+#define LAM_QL 0
+#endif
 constexpr int kTile = LAM_TILE;               // gridding tile edge (fine-grid cells owned by a job)
 constexpr int kTP = LAM_TP;                 // float2 elements per storage row in shared memory (multiple of 16, >= kTile + 2W - 2)
 constexpr int kNU = LAM_NU;                  // samples a lane spreads per step (4*kNU concurrent slots per warp)
@@ -454,7 +457,9 @@ __global__ void __launch_bounds__(32) k_spread(SpreadArgs a) {
             }
             const int nseg = min(n - seg, kStage);
             // 4*kNU slots (kNU per lane) take samples Qe apart; one sweep of Qe steps covers the segment
-            const int Qe = max(Q, (nseg + 4 * kNU - 1) / (4 * kNU));
+            // concurrent samples must be >= W cells apart along the major axis: Q_line = ceil(W / |aM|) (<= Q)
+            const int Ql = LAM_QL ? min(Q, (int)ceilf((float)W / fabsf(aM) + 1e-3f)) : Q;
+            const int Qe = max(Ql, (nseg + 4 * kNU - 1) / (4 * kNU));
 #pragma unroll 1
             for (int it = 0; it < Qe; ++it) {
               float2 acc[kNU][W];
@@ -621,7 +626,8 @@ struct ZArgs {
   size_t zstride;
   const float2* tw;      // length M3
   const float* ztab;     // [M3][KZ]
-  const int* zlo;        // [M3]
+  const int* zlo;        // [M3] first plane with a tap on cell i
+  const int* zcnt;       // [M3] number of such planes (<= KZ)
   const float* zlast;    // [M3]
   const float* dx;       // [n]  1/kaphat(x/M)
   const float* dz;       // [nz] 1/kaphat(x3/M3)
@@ -651,7 +657,8 @@ __global__ void __launch_bounds__(256) k_zstage(ZArgs a) {
     float wl = __ldg(&a.zlast[i]);
     float2 v = Ain[last + t];
     float2 acc = make_float2(v.x * wl, v.y * wl);
-    for (int s = 0; s < KZ; ++s) {
+    const int cnt = __ldg(&a.zcnt[i]);
+    for (int s = 0; s < cnt; ++s) {
       float wv = __ldg(&wt[s]);
       float2 x = ap[s * kZCb];
       acc.x = fmaf(x.x, wv, acc.x);
