@@ -570,7 +570,7 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
       note_launch();
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;
-      size_t sm = ((size_t)(kTile + 2 * W - 2) * kTP + 2 * kStage) * sizeof(float2);
+      size_t sm = ((size_t)(kHalo ? kTile + 2 * W - 2 : kTile) * kTP + 2 * kStage) * sizeof(float2);
       cudaFuncSetAttribute(k_spread<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
       k_spread<W><<<(unsigned)sa.njobs, 32, sm, s>>>(sa);
       note_launch();

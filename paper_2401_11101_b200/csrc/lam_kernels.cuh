@@ -20,8 +20,14 @@ namespace lam {
 
 #ifndef LAM_TILE
 #define LAM_TILE 32
-#define LAM_TP 48
+#define LAM_TP 32
 #define LAM_NU 1
+#endif
+#ifndef LAM_HALO
+#define LAM_HALO 0
+#endif
+#ifndef LAM_UNROLL
+#define LAM_UNROLL 1
 #endif
 #ifndef LAM_QL
 #define LAM_QL 0
@@ -29,6 +35,8 @@ namespace lam {
 constexpr int kTile = LAM_TILE;               // gridding tile edge (fine-grid cells owned by a job)
 constexpr int kTP = LAM_TP;                 // float2 elements per storage row in shared memory (multiple of 16, >= kTile + 2W - 2)
 constexpr int kNU = LAM_NU;                  // samples a lane spreads per step (4*kNU concurrent slots per warp)
+constexpr int kSweepUnroll = LAM_UNROLL;  // unrolling of the slot sweep loop of k_spread
+constexpr bool kHalo = LAM_HALO != 0;    // storage tile with a kernel halo (no per-tap bounds tests) or without
 constexpr int kStage = 64;              // samples of one line segment parked in shared memory
 constexpr int kJobSegs = 32;            // target segments (theta crossings) per job
 constexpr int kJobMaxSpan = 1023;       // max theta span of one job (10 bits)
@@ -364,8 +372,8 @@ __global__ void k_zero_tiles(SpreadArgs a) {
 template <int W>
 __global__ void __launch_bounds__(32) k_spread(SpreadArgs a) {
   extern __shared__ float2 tile[];
-  constexpr int H = W - 1;                           // low-side halo of the storage
-  constexpr int ROWS = kTile + 2 * W - 2;
+  constexpr int H = kHalo ? W - 1 : 0;               // low-side halo of the storage (0: taps are bounds-tested)
+  constexpr int ROWS = kHalo ? kTile + 2 * W - 2 : kTile;
   const SpreadGeom& g = a.g;
   const int Q = g.kstride;  // sample distance between slots (footprints disjoint)
   const int lane = threadIdx.x;
@@ -460,13 +468,14 @@ __global__ void __launch_bounds__(32) k_spread(SpreadArgs a) {
             // concurrent samples must be >= W cells apart along the major axis: Q_line = ceil(W / |aM|) (<= Q)
             const int Ql = LAM_QL ? min(Q, (int)ceilf((float)W / fabsf(aM) + 1e-3f)) : Q;
             const int Qe = max(Ql, (nseg + 4 * kNU - 1) / (4 * kNU));
-#pragma unroll 1
+#pragma unroll kSweepUnroll
             for (int it = 0; it < Qe; ++it) {
               float2 acc[kNU][W];
               float wm[kNU][W];
               float2 vw[kNU];
               unsigned ad[kNU];
               bool ok[kNU];
+              int rw0[kNU];
 #pragma unroll
               for (int u = 0; u < kNU; ++u) {
                 const int kk = (sidx + 4 * u) * Qe + it;
@@ -474,8 +483,10 @@ __global__ void __launch_bounds__(32) k_spread(SpreadArgs a) {
                 const float tM = fmaf(fk, aM, M0), tm = fmaf(fk, am, m0);
                 const float cf = ceilf(tM - 0.5f * W), rf = ceilf(tm - 0.5f * W);
                 const int col0 = (int)cf, row0 = (int)rf;
-                ok[u] = role && kk < nseg && (unsigned)(col0 + H) < (unsigned)(kTile + H) &&
-                        (unsigned)(row0 + H) < (unsigned)(kTile + H);
+                ok[u] = role && kk < nseg && (unsigned)(col0 + W - 1) < (unsigned)(kTile + W - 1) &&
+                        (unsigned)(row0 + W - 1) < (unsigned)(kTile + W - 1);
+                if (!kHalo) ok[u] = ok[u] && (unsigned)(col0 + j1) < (unsigned)kTile;  // this lane's tap column
+                rw0[u] = row0;
                 const float2 v = stg[sb * kStage + (kk & (kStage - 1))];
                 // this lane's tap polynomial at both offsets: its own major-axis weight, and minor-axis weight j1
                 // of the slot's sample, which the W lanes of the slot then exchange
@@ -499,7 +510,7 @@ __global__ void __launch_bounds__(32) k_spread(SpreadArgs a) {
               for (int u = 0; u < kNU; ++u)
 #pragma unroll
                 for (int j2 = 0; j2 < W; ++j2)
-                  if (ok[u]) acc[u][j2] = lds_v(ad[u] + j2 * (kTP * 8));
+                  if (ok[u] && (kHalo || (unsigned)(rw0[u] + j2) < (unsigned)kTile)) acc[u][j2] = lds_v(ad[u] + j2 * (kTP * 8));
 #pragma unroll
               for (int u = 0; u < kNU; ++u)
 #pragma unroll
@@ -511,7 +522,7 @@ __global__ void __launch_bounds__(32) k_spread(SpreadArgs a) {
               for (int u = 0; u < kNU; ++u)
 #pragma unroll
                 for (int j2 = 0; j2 < W; ++j2)
-                  if (ok[u]) sts_v(ad[u] + j2 * (kTP * 8), acc[u][j2]);
+                  if (ok[u] && (kHalo || (unsigned)(rw0[u] + j2) < (unsigned)kTile)) sts_v(ad[u] + j2 * (kTP * 8), acc[u][j2]);
             }
           }
           if (!more) break;
