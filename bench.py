@@ -262,6 +262,15 @@ def run_ours(args):
         ach = model[names[dom]]["bytes"] / (stage[dom] * 1e-3) / 1e9
         roof = {"kernel": names[dom], "stage": names[dom], "bound": "hbm", "achieved": round(ach, 1), "peak": hbm,
                 "unit": "GB/s", "frac": round(ach / hbm, 4), "traffic": None, "peak_source": src}
+    # traffic: dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), if any
+    try:
+        import csv
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "r01_traffic.csv"))):
+            if int(row["config"]) == args.config and row["stage"] == names[dom]:
+                roof["traffic"] = float(row["dram_bytes_per_launch"])
+                roof["traffic_note"] = row["source"]
+    except Exception:
+        pass
     roof["stages"] = stages
     roof["share_of_step"] = round(stage[dom] / max(1e-9, sum(stage[:4])), 4)
     total_bytes = sum(m["bytes"] for m in model.values())
