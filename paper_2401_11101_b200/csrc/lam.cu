@@ -56,6 +56,7 @@ struct lam_plan {
   float2 *d_Pu = nullptr, *d_Pv = nullptr, *d_PuNone = nullptr;
   float2 *d_tw_w = nullptr, *d_tw_h = nullptr, *d_tw_M = nullptr, *d_tw_M3 = nullptr;
   float *d_ztab = nullptr, *d_zlast = nullptr, *d_dx = nullptr, *d_dz = nullptr, *d_dark = nullptr, *d_flat = nullptr;
+  float2* d_df = nullptr;
   int *d_zlo = nullptr, *d_zcnt = nullptr;
   uint2* d_jobs = nullptr;
   std::vector<long long> job_off;  // [NP+1] first job of each plane
@@ -173,7 +174,7 @@ struct Launch {
   }
   static void z(dim3 g, size_t sm, cudaStream_t s, const ZArgs& a) {
     cudaFuncSetAttribute(k_zstage<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    k_zstage<L><<<g, 256, sm, s>>>(a);
+    k_zstage<L><<<g, sm > 100 * 1024 ? 512 : 256, sm, s>>>(a);
       note_launch();
   }
 };
@@ -218,7 +219,7 @@ struct StageScope {
 
 void free_all(lam_plan* p) {
   void* ptrs[] = {p->d_cs,    p->d_Pu,  p->d_Pv,  p->d_PuNone, p->d_tw_w, p->d_tw_h,   p->d_tw_M, p->d_tw_M3,
-                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_zcnt,
+                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_zcnt, p->d_df,
                   p->d_R,     p->d_arena, p->d_G, p->d_T};
   for (void* q : ptrs)
     if (q) cudaFree(q);
@@ -527,6 +528,9 @@ lam_status lam_set_darkflat(lam_plan* p, const float* dark, const float* flat) {
   if (!p->d_flat && (st = dalloc(p, &p->d_flat, cnt)) != LAM_OK) return st;
   CU(p, cudaMemcpy(p->d_dark, dark, cnt * 4, cudaMemcpyDefault));
   CU(p, cudaMemcpy(p->d_flat, flat, cnt * 4, cudaMemcpyDefault));
+  if (!p->d_df && (st = dalloc(p, &p->d_df, cnt)) != LAM_OK) return st;
+  k_darkflat<<<(unsigned)((cnt + 255) / 256), 256>>>(p->d_dark, p->d_flat, p->d_df, cnt);
+  CU(p, cudaDeviceSynchronize());
   p->have_darkflat = true;
   return LAM_OK;
 }
@@ -549,7 +553,7 @@ static bool is_device_ptr(const void* q) {
 // S0 + S1 for projections [th0, th0 + nth) at device pointer `chunk` (the first projection of the chunk)
 static void launch_s1(lam_plan* p, const void* chunk, int th0, int nth, cudaStream_t s) {
   const bool raw = p->prm.input == LAM_INPUT_U16_RAW;
-  RowsArgs ra{chunk, p->d_dark, p->d_flat, p->prm.t_min, p->d_R, p->d_Pu, p->d_tw_w, p->h, p->WR, p->rows_nb};
+  RowsArgs ra{chunk, p->d_df, p->prm.t_min, p->d_R, p->d_Pu, p->d_tw_w, p->h, p->WR, p->rows_nb};
   dim3 gr(p->h / 2 / p->rows_nb, nth);
   size_t smr = (size_t)p->rows_nb * fft_span(p->w) * sizeof(float2);
   DISPATCH_LOG(p->logw, rows(raw, gr, smr, s, ra));

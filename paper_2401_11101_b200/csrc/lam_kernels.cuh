@@ -26,6 +26,9 @@ namespace lam {
 #ifndef LAM_HALO
 #define LAM_HALO 0
 #endif
+#ifndef LAM_SEGS
+#define LAM_SEGS 32
+#endif
 #ifndef LAM_MINB
 #define LAM_MINB 1
 #endif
@@ -41,17 +44,22 @@ constexpr int kNU = LAM_NU;                  // samples a lane spreads per step 
 constexpr int kSweepUnroll = LAM_UNROLL;  // unrolling of the slot sweep loop of k_spread
 constexpr bool kHalo = LAM_HALO != 0;    // storage tile with a kernel halo (no per-tap bounds tests) or without
 constexpr int kStage = 64;              // samples of one line segment parked in shared memory
-constexpr int kJobSegs = 32;            // target segments (theta crossings) per job
+constexpr int kJobSegs = LAM_SEGS;            // target segments (theta crossings) per job
 constexpr int kJobMaxSpan = 1023;       // max theta span of one job (10 bits)
 constexpr int kMaxW = 8;
+
+// (dark, flat) -> (dark, 1 / max(flat - dark, 1)): the per-pixel constants of the -log prep (reading Q12)
+__global__ void k_darkflat(const float* dark, const float* flat, float2* df, size_t cnt) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < cnt) df[i] = make_float2(dark[i], 1.0f / fmaxf(flat[i] - dark[i], 1.0f));
+}
 
 // ---------------------------------------------------------------------------------------------------------------
 // S0 + S1a: rows
 // ---------------------------------------------------------------------------------------------------------------
 struct RowsArgs {
   const void* proj;     // chunk base: [nth][h][w] float or uint16
-  const float* dark;    // [h][w]
-  const float* flat;
+  const float2* df;     // [h][w] (dark, 1 / max(flat - dark, 1))
   float tmin;
   float2* R;            // [nth][h][WR]  filtered half spectra of the rows
   const float2* Pu;     // [w/2+1]  H[k] e^{2 pi i k c_u / w} / (w h)
@@ -70,9 +78,8 @@ __global__ void __launch_bounds__(256) k_rows(RowsArgs a) {
     if (RAW) {
       const uint16_t* p = (const uint16_t*)a.proj + pbase + (size_t)jv * w + ju;
       float r0 = (float)p[0], r1 = (float)p[w];
-      float d0 = __ldg(&a.dark[jv * w + ju]), d1 = __ldg(&a.dark[(jv + 1) * w + ju]);
-      float f0 = __ldg(&a.flat[jv * w + ju]), f1 = __ldg(&a.flat[(jv + 1) * w + ju]);
-      float t0 = (r0 - d0) / fmaxf(f0 - d0, 1.0f), t1 = (r1 - d1) / fmaxf(f1 - d1, 1.0f);
+      const float2 g0 = __ldg(&a.df[jv * w + ju]), g1 = __ldg(&a.df[(jv + 1) * w + ju]);
+      float t0 = (r0 - g0.x) * g0.y, t1 = (r1 - g1.x) * g1.y;
       return make_float2(-logf(fmaxf(t0, a.tmin)), -logf(fmaxf(t1, a.tmin)));
     } else {
       const float* p = (const float*)a.proj + pbase + (size_t)jv * w + ju;
@@ -651,7 +658,7 @@ struct ZArgs {
 };
 
 template <int LOGM3>
-__global__ void __launch_bounds__(256) k_zstage(ZArgs a) {
+__global__ void __launch_bounds__(512) k_zstage(ZArgs a) {
   constexpr int M3 = 1 << LOGM3, P = fft_tfast_pitch(M3, kZCb);
   extern __shared__ float2 sm[];
   float2* Gz = sm;                                // [8][P]
