@@ -43,6 +43,18 @@ __host__ __device__ constexpr int fft_span(int n) { return n <= 256 ? n + (n >> 
 // shared-memory pitch of a TFAST block_fft: a multiple of 16 plus 16/nb (nb <= 16 transforms) or 1
 __host__ __device__ constexpr int fft_tfast_pitch(int n, int nb) { return ((fft_span(n) + 15) & ~15) + (nb >= 16 ? 1 : 16 / nb); }
 
+// swizzle constant of logical position p (three- and four-pass sizes): depends on the leading digit of p and, for
+// four-pass sizes, on the lowest bit of the second digit only, so one evaluation serves a whole work item
+template <int LOGN>
+__device__ __forceinline__ int fft_xor(int p) {
+  using F = FftShape<LOGN>;
+  const int d0 = p >> F::sb(0);
+  int x = (int)(__brev((unsigned)d0) >> 28);
+  if constexpr (F::rb(0) == 3) x ^= d0 & 1;
+  if constexpr (F::NP == 4) x ^= ((p >> F::sb(1)) & 1) << 3;
+  return x;
+}
+
 // physical index of logical position p of a transform
 template <int LOGN>
 __device__ __forceinline__ int fft_swz(int p) {
@@ -50,11 +62,19 @@ __device__ __forceinline__ int fft_swz(int p) {
   if constexpr (F::NP <= 2) {
     return p + (p >> 4);
   } else {
-    const int d0 = p >> F::sb(0);
-    int x = (int)(__brev((unsigned)d0) >> 28);
-    if constexpr (F::rb(0) == 3) x ^= d0 & 1;
-    if constexpr (F::NP == 4) x ^= ((p >> F::sb(1)) & 1) << 3;
-    return p ^ x;
+    return p ^ fft_xor<LOGN>(p);
+  }
+}
+
+// physical index of position base + off of a work item whose swizzle constant xb was taken at `base`; `flip8` toggles
+// swizzle bit 3 (pass 1 of four-pass sizes, where the element index k walks the second digit: flip8 = k & 1)
+template <int LOGN>
+__device__ __forceinline__ int fft_swz_item(int base, int off, int xb, bool flip8 = false) {
+  using F = FftShape<LOGN>;
+  if constexpr (F::NP <= 2) {
+    return (base + off) + ((base + off) >> 4);
+  } else {
+    return (base + off) ^ (flip8 ? xb ^ 8 : xb);
   }
 }
 
@@ -152,12 +172,14 @@ __device__ __forceinline__ void fft_mid_passes(float2* s, int nb, int lognb, int
       fft_split<TFAST>(it, IB, lognb, t, u);
       const int j = u & (S - 1), base = ((u >> SB) << (SB + RB)) | j;
       float2* st = s + t * pitch;
+      const int xb = F::NP > 2 ? fft_xor<LOGN>(base) : 0;
+      constexpr bool WALK2 = F::NP == 4 && I == 1;  // the element index walks the second digit
       float2 a[R];
 #pragma unroll
-      for (int k = 0; k < R; ++k) a[k] = st[fft_swz<LOGN>(base + k * S)];
+      for (int k = 0; k < R; ++k) a[k] = st[fft_swz_item<LOGN>(base, k * S, xb, WALK2 && (k & 1))];
       fft_bfly<LOGN, DIR, I>(a, j, tw);
 #pragma unroll
-      for (int q = 0; q < R; ++q) st[fft_swz<LOGN>(base + q * S)] = a[brev_bits(q, RB)];
+      for (int q = 0; q < R; ++q) st[fft_swz_item<LOGN>(base, q * S, xb, WALK2 && (q & 1))] = a[brev_bits(q, RB)];
     }
     __syncthreads();
     fft_mid_passes<LOGN, DIR, TFAST, I + 1>(s, nb, lognb, pitch, tw);
@@ -184,8 +206,16 @@ __device__ __forceinline__ void block_fft(float2* s, int nb, int lognb, int pitc
       for (int k = 0; k < R; ++k) a[k] = ld(t, u + k * S);
       fft_bfly<LOGN, DIR, 0>(a, u, tw);
       float2* sp = s + t * pitch;
+      // leading digit = q: the swizzle constant is a compile-time value (plus one bit of u for four-pass sizes)
 #pragma unroll
-      for (int q = 0; q < R; ++q) sp[fft_swz<LOGN>(u + q * S)] = a[brev_bits(q, RB)];
+      for (int q = 0; q < R; ++q) {
+        if constexpr (F::NP <= 2) {
+          sp[fft_swz<LOGN>(u + q * S)] = a[brev_bits(q, RB)];
+        } else {
+          const int x = fft_xor<LOGN>((q << SB) | (F::NP == 4 ? (u & (1 << F::sb(1))) : 0));
+          sp[(u ^ x) + q * S] = a[brev_bits(q, RB)];
+        }
+      }
     }
     __syncthreads();
   }
@@ -207,16 +237,17 @@ __device__ __forceinline__ void block_fft(float2* s, int nb, int lognb, int pitc
         sh += F::rb(i);
       }
       float2* sp = s + t * pitch;
+      const int xb = F::NP > 2 ? fft_xor<LOGN>(base) : 0;
       float2 a[R];
 #pragma unroll
-      for (int k = 0; k < R; ++k) a[k] = sp[fft_swz<LOGN>(base + k)];
+      for (int k = 0; k < R; ++k) a[k] = sp[fft_swz_item<LOGN>(base, k, xb)];
       fft_reg<R, DIR>(a);
       if constexpr (SINK) {
 #pragma unroll
         for (int q = 0; q < R; ++q) st(t, v + (q << IB), a[brev_bits(q, RB)]);
       } else {
 #pragma unroll
-        for (int q = 0; q < R; ++q) sp[fft_swz<LOGN>(base + q)] = a[brev_bits(q, RB)];
+        for (int q = 0; q < R; ++q) sp[fft_swz_item<LOGN>(base, q, xb)] = a[brev_bits(q, RB)];
       }
     }
     if constexpr (!SINK) __syncthreads();
