@@ -97,8 +97,10 @@ lam_status lam_set_darkflat(lam_plan* plan, const float* dark, const float* flat
  * pointer kinds and stream semantics. */
 lam_status lam_backproject(lam_plan* plan, const void* proj, float* vol, void* cuda_stream);
 
-/* proj <- L vol (overwrites proj, float32), the transpose of lam_backproject with filter none (the plan's filter
- * setting is ignored).  Device pointers only.  Not tuned: it exists for the adjoint identity. */
+/* proj <- L vol (overwrites proj, float32): Eq. 5 as the exact transpose, stage by stage in reverse
+ * order, of lam_backproject with filter none (the plan's filter setting is ignored; an input plan of type uint16
+ * still yields float32 line integrals).  Device pointers only (host pointers: LAM_EUNSUPPORTED); asynchronous on
+ * cuda_stream.  <L f, d> = <f, L* d> holds to fp32 rounding (about 1e-6 relative).  Not tuned. */
 lam_status lam_forward(lam_plan* plan, const float* vol, float* proj, void* cuda_stream);
 
 /* Per-stage device times of the LAST lam_backproject, milliseconds, measured with CUDA events on the plan's

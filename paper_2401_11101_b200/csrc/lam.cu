@@ -18,6 +18,7 @@
 
 #include "../../include/lam.h"
 #include "lam_kernels.cuh"
+#include "lam_forward.cuh"
 
 using namespace lam;
 
@@ -57,6 +58,8 @@ struct lam_plan {
   float2 *d_tw_w = nullptr, *d_tw_h = nullptr, *d_tw_M = nullptr, *d_tw_M3 = nullptr;
   float *d_ztab = nullptr, *d_zlast = nullptr, *d_dx = nullptr, *d_dz = nullptr, *d_dark = nullptr, *d_flat = nullptr;
   float2* d_df = nullptr;
+  float* d_wz = nullptr;  // [NP][W] x3 tap weights per plane (lam_forward)
+  int* d_bz = nullptr;    // [NP] first x3 tap per plane
   int *d_zlo = nullptr, *d_zcnt = nullptr;
   uint2* d_jobs = nullptr;
   std::vector<long long> job_off;  // [NP+1] first job of each plane
@@ -172,6 +175,31 @@ struct Launch {
     k_ifft_x2<L><<<g, threads, sm, s>>>(a);
       note_launch();
   }
+  static void zT(dim3 g, size_t sm, cudaStream_t s, const ZTArgs& a) {
+    cudaFuncSetAttribute(k_zstage_T<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_zstage_T<L><<<g, 256, sm, s>>>(a);
+    note_launch();
+  }
+  static void x2T(dim3 g, int threads, size_t sm, cudaStream_t s, const IfftArgs& a) {
+    cudaFuncSetAttribute(k_fft_x2_T<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_fft_x2_T<L><<<g, threads, sm, s>>>(a);
+    note_launch();
+  }
+  static void x1T(dim3 g, size_t sm, cudaStream_t s, const IfftArgs& a) {
+    cudaFuncSetAttribute(k_fft_x1_T<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_fft_x1_T<L><<<g, 256, sm, s>>>(a);
+    note_launch();
+  }
+  static void colsT(dim3 g, int threads, size_t sm, cudaStream_t s, const ColsTArgs& a) {
+    cudaFuncSetAttribute(k_cols_T<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_cols_T<L><<<g, threads, sm, s>>>(a);
+    note_launch();
+  }
+  static void rowsT(dim3 g, size_t sm, cudaStream_t s, const RowsTArgs& a) {
+    cudaFuncSetAttribute(k_rows_T<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_rows_T<L><<<g, 256, sm, s>>>(a);
+    note_launch();
+  }
   static void z(dim3 g, size_t sm, cudaStream_t s, const ZArgs& a) {
     cudaFuncSetAttribute(k_zstage<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     k_zstage<L><<<g, sm > 100 * 1024 ? 512 : 256, sm, s>>>(a);
@@ -219,7 +247,7 @@ struct StageScope {
 
 void free_all(lam_plan* p) {
   void* ptrs[] = {p->d_cs,    p->d_Pu,  p->d_Pv,  p->d_PuNone, p->d_tw_w, p->d_tw_h,   p->d_tw_M, p->d_tw_M3,
-                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_zcnt, p->d_df,
+                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_zcnt, p->d_df, p->d_wz, p->d_bz,
                   p->d_R,     p->d_arena, p->d_G, p->d_T};
   for (void* q : ptrs)
     if (q) cudaFree(q);
@@ -351,14 +379,17 @@ lam_status make_tables(lam_plan* p) {
     int KZ = 1;
     for (int i = 0; i < M3; ++i) KZ = std::max(KZ, hi[i] - lo[i] + 1);
     p->KZ = KZ;
-    std::vector<float> ztab((size_t)M3 * KZ, 0.f), zlast(M3, 0.f);
+    std::vector<float> ztab((size_t)M3 * KZ, 0.f), zlast(M3, 0.f), wz((size_t)NP * W);
+    std::vector<int> bz(NP);
     for (int q = 0; q <= h / 2; ++q) {
       int kv = q == h / 2 ? -h / 2 : q;
       double t3 = (double)M3 * kv * cphi / h;
       int b = (int)std::ceil(t3 - 0.5 * W);
+      bz[q] = b;
       for (int j = 0; j < W; ++j) {
         int i = cell(b + j);
         float wv = (float)p->gk.kap(t3 - (b + j));
+        wz[(size_t)q * W + j] = wv;
         if (q == h / 2) zlast[i] += wv;
         else ztab[(size_t)i * KZ + (q - lo[i])] += wv;
       }
@@ -369,6 +400,8 @@ lam_status make_tables(lam_plan* p) {
     if ((st = upload(p, &p->d_zlo, lo)) != LAM_OK) return st;
     if ((st = upload(p, &p->d_zcnt, cnt)) != LAM_OK) return st;
     if ((st = upload(p, &p->d_zlast, zlast)) != LAM_OK) return st;
+    if ((st = upload(p, &p->d_wz, wz)) != LAM_OK) return st;
+    if ((st = upload(p, &p->d_bz, bz)) != LAM_OK) return st;
   }
   std::vector<float> dx(n), dz(nz);
   for (int i = 0; i < n; ++i) dx[i] = (float)(1.0 / p->gk.kaphat((double)(i - n / 2) / M));
@@ -701,9 +734,52 @@ lam_status lam_backproject(lam_plan* p, const void* proj, float* vol, void* cuda
 }
 
 lam_status lam_forward(lam_plan* p, const float* vol, float* proj, void* cuda_stream) {
-  (void)vol; (void)proj; (void)cuda_stream;
   if (!p) return LAM_EINVAL;
-  return fail(p, LAM_EUNSUPPORTED, "lam_forward is not implemented in this build");
+  if (!vol || !proj) return fail(p, LAM_EINVAL, "vol / proj is NULL");
+  cudaSetDevice(p->device);
+  if (!is_device_ptr(vol) || !is_device_ptr(proj)) return fail(p, LAM_EUNSUPPORTED, "lam_forward takes device pointers only");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  p->launches = 0;
+  g_launch_error = cudaSuccess;
+  p->stage_valid = false;
+  const int n = p->n, M = p->M, NP = p->NP;
+  // (x3 stage)^T: all columns -> A^T[p][x2][x1]
+  {
+    ZTArgs za{vol, p->d_A, p->d_tw_M3, p->d_wz, p->d_bz, p->d_dx, p->d_dz, n, p->nz, NP, p->W};
+    size_t sm = (size_t)kZCb * fft_tfast_pitch(p->M3, kZCb) * sizeof(float2);
+    DISPATCH_LOG(p->logM3, zT(dim3(n / kZCb, n), sm, s, za));
+    p->launches += 1;
+  }
+  // planes, last batch first (the spectra planes are written right-aligned into the arena the A^T planes leave)
+  for (int p0 = ((NP - 1) / p->PB) * p->PB; p0 >= 0; p0 -= p->PB) {
+    const int np = std::min(p->PB, NP - p0), nb2 = 1 << p->x2_lnb;
+    IfftArgs a2{p->d_A + (size_t)p0 * n * n, p->d_T, p->d_tw_M, n, nb2, p->x2_lnb};
+    DISPATCH_LOG(p->logM, x2T(dim3(n / nb2, np), (size_t)nb2 * M >= 16384 ? 512 : 256,
+                              (size_t)nb2 * fft_tfast_pitch(M, nb2) * sizeof(float2), s, a2));
+    IfftArgs a1{p->d_T, p->d_G, p->d_tw_M, n, p->x1_nb, 0};
+    DISPATCH_LOG(p->logM, x1T(dim3(M / p->x1_nb, np), (size_t)p->x1_nb * fft_span(M) * sizeof(float2), s, a1));
+    GatherArgs ga{p->geom, p->kp, p->d_G, p->d_S, p->WQ, p0, np};
+    dispatch_W(p->W, [&](auto Wc) {
+      constexpr int W = decltype(Wc)::value;
+      k_gather<W><<<dim3((p->w + 1 + 255) / 256, p->ntheta, np), 256, 0, s>>>(ga);
+      note_launch();
+    });
+    p->launches += 3;
+  }
+  // (S1)^T: un-fold + inverse FFT along v, then inverse FFT along u; H = 1 (the filter is not part of L)
+  const int cb = 1 << p->cols_lcb, nbr = std::max(1, std::min(p->h, 4096 / p->w));
+  for (int th0 = 0; th0 < p->ntheta; th0 += p->TC) {
+    const int nth = std::min(p->TC, p->ntheta - th0);
+    ColsTArgs ca{p->d_S, p->d_R, p->d_Pv, p->d_tw_h, p->w, p->WR, p->WQ, p->ntheta, th0, p->cols_lcb};
+    DISPATCH_LOG(p->logh, colsT(dim3((p->w / 2 + 1 + cb - 1) / cb, nth), (size_t)cb * p->h >= 16384 ? 512 : 256,
+                                (size_t)cb * fft_tfast_pitch(p->h, cb) * sizeof(float2), s, ca));
+    RowsTArgs ra{p->d_R, proj + (size_t)th0 * p->h * p->w, p->d_PuNone, p->d_tw_w, p->h, p->WR, nbr};
+    DISPATCH_LOG(p->logw, rowsT(dim3(p->h / nbr, nth), (size_t)nbr * fft_span(p->w) * sizeof(float2), s, ra));
+    p->launches += 2;
+  }
+  CU(p, cudaGetLastError());
+  if (g_launch_error != cudaSuccess) return fail(p, LAM_ECUDA, "kernel launch failed: %s", cudaGetErrorString(g_launch_error));
+  return LAM_OK;
 }
 
 lam_status lam_stage_ms(lam_plan* p, float ms[6]) {

@@ -1,0 +1,224 @@
+// lam_forward.cuh — kernels of lam_forward: proj = L vol, the exact transpose (over the reals) of lam_backproject
+// with filter = none, stage by stage in reverse order (Eq. 5: L = F*_2D F_u3D; the USFFT steps of
+// PAPER.md:136-138 in their forward order: division by the kernel transform, FFT, convolution-type interpolation).
+// Not tuned: it exists for the adjoint identity <L f, d> = <f, L* d> and as the forward model of iterative schemes.
+//
+//   k_zstage_T   (x3 stage)^T    vol * deapodisation -> zero-pad -> forward FFT along x3 -> interpolate at t3(k_v)
+//   k_fft_x2_T   (k_ifft_x2)^T   zero-pad x2 (with the centring signs) -> forward FFT
+//   k_fft_x1_T   (k_ifft_x1)^T   zero-pad x1 -> forward FFT                     -> fine-grid plane G^T
+//   k_gather     (k_spread)^T    S^T[p][theta][q] = sum of W x W taps of G^T at the sample position (Eq. 6)
+//   k_cols_T     (k_cols)^T      un-fold the k_v >= 0 planes onto all h rows, inverse FFT along v
+//   k_rows_T     (k_rows)^T      conj(Pu) * half spectrum -> inverse FFT along u -> real part
+//
+// Transposition rules used: a complex-linear map F becomes F^H (an unnormalised FFT of direction D becomes the
+// unnormalised FFT of direction -D); y = Re(x) becomes x = y + 0i; g -> b conj(g) becomes s -> b conj(s); real
+// weights stay.
+#pragma once
+#include "lam_kernels.cuh"
+
+namespace lam {
+
+struct ZTArgs {
+  const float* vol;      // [nz][n][n]
+  float2* A;             // [h/2+1][n][n]
+  const float2* tw;      // length M3
+  const float* wz;       // [h/2+1][W] tap weights of plane p
+  const int* bz;         // [h/2+1] first tap m3 of plane p
+  const float* dx;       // [n]
+  const float* dz;       // [nz]
+  int n, nz, np, W;
+};
+
+template <int LOGM3>
+__global__ void __launch_bounds__(256) k_zstage_T(ZTArgs a) {
+  constexpr int M3 = 1 << LOGM3, P = fft_tfast_pitch(M3, kZCb);
+  extern __shared__ float2 sm[];
+  const int ix2 = blockIdx.y, c0 = blockIdx.x * kZCb;
+  const size_t nn = (size_t)a.n * a.n;
+  const int hz = a.nz / 2;
+  const float dx2 = a.dx[ix2];
+  const float* vb = a.vol + (size_t)ix2 * a.n + c0;
+  auto ld = [&](int t, int k) -> float2 {  // bin k of the zero-padded column: x3 = k (k < nz/2) or k - M3
+    if (k >= hz && k < M3 - hz) return make_float2(0.f, 0.f);
+    const int ix3 = k < hz ? k + hz : k - (M3 - hz);
+    return make_float2(vb[(size_t)ix3 * nn + t] * a.dz[ix3] * dx2 * a.dx[c0 + t], 0.f);
+  };
+  block_fft<LOGM3, -1, true, false>(sm, kZCb, kZLog, P, a.tw, ld, [](int, int, float2) {});
+  float2* Ab = a.A + (size_t)ix2 * a.n + c0;
+  for (int idx = threadIdx.x; idx < a.np * kZCb; idx += blockDim.x) {
+    const int p = idx >> kZLog, c = idx & (kZCb - 1);
+    const int b = a.bz[p];
+    float2 acc = make_float2(0.f, 0.f);
+    for (int j = 0; j < a.W; ++j) {
+      const float2 v = sm[c * P + fft_at<LOGM3>((b + j) & (M3 - 1))];
+      const float wv = a.wz[p * a.W + j];
+      acc.x = fmaf(v.x, wv, acc.x);
+      acc.y = fmaf(v.y, wv, acc.y);
+    }
+    Ab[(size_t)p * nn + c] = acc;
+  }
+}
+
+// (k_ifft_x2)^T: T^T[pl][i2][ix1] = sum_{kept k} e^{-2 pi i k i2/M} (-1)^k A^T[pl][ix(k)][ix1]
+template <int LOGM>
+__global__ void __launch_bounds__(512) k_fft_x2_T(IfftArgs a) {
+  constexpr int M = 1 << LOGM;
+  extern __shared__ float2 sm[];
+  const int P = fft_tfast_pitch(M, a.nb);
+  const int pl = blockIdx.y, c0 = blockIdx.x * a.nb;
+  const int n = a.n, hn = a.n / 2;
+  const float2* in = a.in + (size_t)pl * n * n + c0;   // A^T plane [n][n]
+  float2* out = a.out + (size_t)pl * M * n + c0;       // T^T plane [M][n]
+  auto ld = [&](int t, int k) -> float2 {
+    if (k >= hn && k < M - hn) return make_float2(0.f, 0.f);
+    const int ix = k < hn ? k + hn : k - (M - hn);
+    float2 v = in[(size_t)ix * n + t];
+    if (k & 1) { v.x = -v.x; v.y = -v.y; }
+    return v;
+  };
+  auto st = [&](int t, int i, float2 v) { out[(size_t)i * n + t] = v; };
+  block_fft<LOGM, -1, true, true>(sm, a.nb, a.lnb, P, a.tw, ld, st);
+}
+
+// (k_ifft_x1)^T: G^T[pl][i2][i1] = sum_{kept k} e^{-2 pi i k i1/M} (-1)^k T^T[pl][i2][ix(k)]
+template <int LOGM>
+__global__ void __launch_bounds__(256) k_fft_x1_T(IfftArgs a) {
+  constexpr int M = 1 << LOGM, P = fft_span(M);
+  extern __shared__ float2 sm[];
+  const int pl = blockIdx.y, r0 = blockIdx.x * a.nb;
+  const int n = a.n, hn = a.n / 2;
+  const float2* in = a.in + ((size_t)pl * M + r0) * n;   // T^T rows [M][n]
+  float2* out = a.out + ((size_t)pl * M + r0) * M;       // G^T rows [M][M]
+  auto ld = [&](int t, int k) -> float2 {
+    if (k >= hn && k < M - hn) return make_float2(0.f, 0.f);
+    const int ix = k < hn ? k + hn : k - (M - hn);
+    float2 v = in[(size_t)t * n + ix];
+    if (k & 1) { v.x = -v.x; v.y = -v.y; }
+    return v;
+  };
+  auto st = [&](int t, int i, float2 v) { out[(size_t)t * M + i] = v; };
+  block_fft<LOGM, -1, false, true>(sm, a.nb, 0, P, a.tw, ld, st);
+}
+
+// (k_spread)^T: one thread per sample (theta, q) of plane p; the same positions, taps and periodic wrap as the
+// spreading (Eq. 6 times M; taps ceil(t - W/2) .. + W - 1; index (m + M/2) mod M)
+struct GatherArgs {
+  SpreadGeom g;
+  KerPoly kp;
+  const float2* G;   // [planes in batch][M][M]
+  float2* S;         // [h/2+1][ntheta][WQ]
+  int WQ, p0, np;
+};
+
+template <int W>
+__global__ void __launch_bounds__(256) k_gather(GatherArgs a) {
+  const SpreadGeom& g = a.g;
+  const int q = blockIdx.x * blockDim.x + threadIdx.x, th = blockIdx.y, pl = blockIdx.z;
+  if (q > g.w) return;
+  const int p = a.p0 + pl, kv = p == g.hh ? -g.hh : p, ku = q - g.w / 2;
+  const double2 cs = g.cs[th];
+  const double rho = g.rho_unit * kv, u = (double)g.a1 * ku;
+  const double t1d = u * cs.x + rho * cs.y, t2d = u * cs.y - rho * cs.x;
+  const double c1 = ceil(t1d - 0.5 * W), c2 = ceil(t2d - 0.5 * W);
+  float w1[W], w2[W];
+  kernel_weights<W>(a.kp, (float)(t1d - c1 - (0.5 * W - 0.5)), w1);
+  kernel_weights<W>(a.kp, (float)(t2d - c2 - (0.5 * W - 0.5)), w2);
+  const int M = g.M, m1 = (int)c1 + M / 2, m2 = (int)c2 + M / 2;
+  const float2* Gp = a.G + (size_t)pl * M * M;
+  float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+  for (int j2 = 0; j2 < W; ++j2) {
+    const float2* row = Gp + (size_t)((m2 + j2) & (M - 1)) * M;
+    float2 r = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int j1 = 0; j1 < W; ++j1) {
+      const float2 v = row[(m1 + j1) & (M - 1)];
+      r.x = fmaf(v.x, w1[j1], r.x);
+      r.y = fmaf(v.y, w1[j1], r.y);
+    }
+    acc.x = fmaf(r.x, w2[j2], acc.x);
+    acc.y = fmaf(r.y, w2[j2], acc.y);
+  }
+  a.S[((size_t)p * g.ntheta + th) * a.WQ + q] = acc;
+}
+
+// (k_cols)^T: for column k_u = k >= 0 of projection theta, C^T[p], p = 0..h-1, from the planes 0..h/2:
+//   k_cols wrote  S[p][hw+k] = a_p C[p],  S[p][hw-k] = b_p conj(C[(h-p) mod h])  (k > 0),  a_p = Pv[p] wplus, b_p = Pv[p] wminus
+//   so            C^T[p] = [p <= h/2] conj(a_p) S^T[p][hw+k] + [p' <= h/2, k > 0] b_p' conj(S^T[p'][hw-k]),  p' = (h-p) mod h
+// then R^T[jv][k] = sum_p e^{+2 pi i p jv/h} C^T[p].
+struct ColsTArgs {
+  const float2* S;   // [h/2+1][ntheta][WQ]
+  float2* R;         // [nth][h][WR]
+  const float2* Pv;
+  const float2* tw;
+  int w, WR, WQ, ntheta, th0, lcb;
+};
+
+template <int LOGH>
+__global__ void __launch_bounds__(512) k_cols_T(ColsTArgs a) {
+  constexpr int h = 1 << LOGH;
+  extern __shared__ float2 sm[];
+  const int cb = 1 << a.lcb, P = fft_tfast_pitch(h, cb);
+  const int thl = blockIdx.y, k0 = blockIdx.x * cb, hw = a.w / 2, th = a.th0 + thl;
+  const int nc = min(cb, hw + 1 - k0);
+  auto wts = [&](int p, int k, float& wplus, float& wminus) {
+    const bool mid = p > 0 && p < h / 2;
+    wplus = mid ? (k < hw ? 2.f : 1.f) : (k < hw ? 1.f : 0.f);
+    wminus = mid ? (k < hw ? 2.f : 1.f) : 1.f;
+  };
+  auto ld = [&](int t, int p) -> float2 {
+    float2 acc = make_float2(0.f, 0.f);
+    if (t >= nc) return acc;
+    const int k = k0 + t;
+    if (p <= h / 2) {
+      float wp, wm;
+      wts(p, k, wp, wm);
+      const float2 s = a.S[((size_t)p * a.ntheta + th) * a.WQ + hw + k], pv = a.Pv[p];
+      const float2 ca = make_float2(pv.x * wp, -pv.y * wp);  // conj(a_p)
+      acc = cmul(ca, s);
+    }
+    const int pp = (h - p) & (h - 1);
+    if (pp <= h / 2 && k > 0) {
+      float wp, wm;
+      wts(pp, k, wp, wm);
+      float2 s = a.S[((size_t)pp * a.ntheta + th) * a.WQ + hw - k];
+      s.y = -s.y;
+      const float2 pv = a.Pv[pp], b = make_float2(pv.x * wm, pv.y * wm);
+      acc = cadd(acc, cmul(b, s));
+    }
+    return acc;
+  };
+  float2* Rb = a.R + (size_t)thl * h * a.WR + k0;
+  auto st = [&](int t, int jv, float2 v) {
+    if (t < nc) Rb[(size_t)jv * a.WR + t] = v;
+  };
+  block_fft<LOGH, +1, true, true>(sm, cb, a.lcb, P, a.tw, ld, st);
+}
+
+// (k_rows)^T: d^T[jv][ju] = Re sum_{k=0}^{w/2} conj(Pu[k]) R^T[jv][k] e^{+2 pi i k ju/w}
+struct RowsTArgs {
+  const float2* R;   // [nth][h][WR]
+  float* proj;       // chunk base [nth][h][w]
+  const float2* Pu;  // [w/2+1]
+  const float2* tw;
+  int h, WR, nb;     // nb rows per block
+};
+
+template <int LOGW>
+__global__ void __launch_bounds__(256) k_rows_T(RowsTArgs a) {
+  constexpr int w = 1 << LOGW, P = fft_span(w);
+  extern __shared__ float2 sm[];
+  const int th = blockIdx.y, r0 = blockIdx.x * a.nb;
+  const float2* Rb = a.R + ((size_t)th * a.h + r0) * a.WR;
+  float* out = a.proj + ((size_t)th * a.h + r0) * w;
+  auto ld = [&](int t, int k) -> float2 {
+    if (k > w / 2) return make_float2(0.f, 0.f);
+    float2 pu = a.Pu[k];
+    pu.y = -pu.y;
+    return cmul(pu, Rb[(size_t)t * a.WR + k]);
+  };
+  auto st = [&](int t, int ju, float2 v) { out[(size_t)t * w + ju] = v.x; };
+  block_fft<LOGW, +1, false, true>(sm, a.nb, 0, P, a.tw, ld, st);
+}
+
+}  // namespace lam

@@ -181,3 +181,40 @@ def test_long_transform_lengths_against_exact_columns(n, nz, h, w, nth):
     ref = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy(), cols=cols)
     got = np.stack([vol[:, c[1], c[0]] for c in cols])
     assert rel(got, ref) <= GATE_TINY
+
+
+def test_forward_against_exact_oracle():
+    """lam_forward = L (Eq. 5) against the oracle's exact forward NUDFT O1 on a small volume."""
+    n, nz, h, w, nth = 32, 32, 32, 32, 8
+    rng = np.random.default_rng(3)
+    zz, yy, xx = np.meshgrid(np.arange(nz) - nz / 2, np.arange(n) - n / 2, np.arange(n) - n / 2, indexing="ij")
+    f = np.zeros((nz, n, n))
+    for _ in range(6):
+        c = rng.uniform(-6, 6, 3)
+        s = rng.uniform(1.5, 3.0)
+        f += rng.uniform(0.5, 1.0) * np.exp(-((xx - c[0]) ** 2 + (yy - c[1]) ** 2 + (zz - c[2]) ** 2) / (2 * s * s))
+    theta = 2 * np.pi * np.arange(nth) / nth + 0.1
+    phi = math.radians(20.0)
+    plan = lam.Plan(n, h, w, theta, phi, nz=nz, filter="none")
+    got = plan.forward(torch.from_numpy(f.astype(np.float32)).cuda()).cpu().numpy()
+    plan.close()
+    ref = O.forward_nudft(O.Geometry(n, h, w, theta, phi, nz=nz, filter="none"), f.astype(np.float32).astype(np.float64))
+    assert rel(got, ref) <= GATE_TINY
+
+
+@pytest.mark.parametrize("idx,n", [(2, 128), (4, 128)])
+def test_adjoint_identity_on_the_gpu(idx, n):
+    """<L f, d> = <f, L* d> for lam_forward / lam_backproject(filter = none): exact transposes stage by stage;
+    SURVEY.md 8(c) gate 1e-5 in fp32 (dot products accumulated in fp64 on the host)."""
+    cfg = inputs.scaled(idx, n)
+    rng = np.random.default_rng(17)
+    f = torch.from_numpy(rng.standard_normal((cfg.nz, cfg.n, cfg.n)).astype(np.float32)).cuda()
+    d = torch.from_numpy(rng.standard_normal((cfg.ntheta, cfg.h, cfg.w)).astype(np.float32)).cuda()
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz, filter="none", plane_batch=7, theta_chunk=11)
+    Lf = plan.forward(f)
+    Ld = plan.backproject(d)
+    torch.cuda.synchronize()
+    plan.close()
+    lhs = float((Lf.double() * d.double()).sum())
+    rhs = float((f.double() * Ld.double()).sum())
+    assert abs(lhs - rhs) <= 1e-5 * abs(lhs), (lhs, rhs)
