@@ -29,6 +29,9 @@ namespace lam {
 #ifndef LAM_SEGS
 #define LAM_SEGS 32
 #endif
+#ifndef LAM_KBOUNDS
+#define LAM_KBOUNDS __launch_bounds__(32)
+#endif
 #ifndef LAM_UNROLL
 #define LAM_UNROLL 1
 #endif
@@ -377,7 +380,7 @@ __global__ void k_zero_tiles(SpreadArgs a) {
 // two runs of 6 contiguous cells of a half-warp sit 7..10 columns apart in rows whose pitch is a multiple of 16:
 // 12 distinct banks per 128-byte wavefront, no conflicts by construction.
 template <int W>
-__global__ void __launch_bounds__(32) k_spread(SpreadArgs a) {
+__global__ void LAM_KBOUNDS k_spread(SpreadArgs a) {
   extern __shared__ float2 tile[];
   constexpr int H = kHalo ? W - 1 : 0;               // low-side halo of the storage (0: taps are bounds-tested)
   constexpr int ROWS = kHalo ? kTile + 2 * W - 2 : kTile;
