@@ -141,6 +141,21 @@ def cpu_sample(cfg, d, nangles, nslices=1, theta=None, mult=3):
                       f"whole job = nz*(t_fix + ntheta*t_angle) extrapolated"}
 
 
+def max_over_ranks(ms, world, device):
+    """Replicas: the job's time is the slowest rank's (MAX all-reduce; identity at world = 1)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gvoxels(world, voxels_per_rank, ms_step):
+    """N independent scans (one per rank, weak scaling) finished in ms_step: aggregate GVoxel/s."""
+    return world * voxels_per_rank / (ms_step * 1e-3) / 1e9
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -200,12 +215,9 @@ def run_ours(args):
     plan.set_profiling(False)
     stage = [s / args.steps for s in stage]
     clocks = sampler.stop() if rank == 0 else None
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
+    ms = max_over_ranks(ms, world, "cuda")
     ms_step = ms / args.steps
-    value = world * cfg.voxels / (ms_step * 1e-3) / 1e9
+    value = whole_job_gvoxels(world, cfg.voxels, ms_step)
 
     # ---- e2e: the same call with host (pinned) buffers; H2D + D2H inside the timed region
     e2e = None
@@ -225,12 +237,9 @@ def run_ours(args):
         barrier()
         wall = (time.perf_counter() - t0) * 1e3
         ems = max(e0.elapsed_time(e1), wall if world == 1 else 0.0)
-        t = torch.tensor([ems], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ems = float(t.item()) / ksteps
+        ems = max_over_ranks(ems, world, "cuda") / ksteps
         err = float((hvol.cuda() - vol).norm() / vol.norm())
-        e2e = {"value": world * cfg.voxels / (ems * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": ems, "steps": ksteps,
+        e2e = {"value": whole_job_gvoxels(world, cfg.voxels, ems), "unit": UNIT, "ms_per_step": ems, "steps": ksteps,
                "h2d_bytes_per_step": hproj.numel() * hproj.element_size(),
                "d2h_bytes_per_step": hvol.numel() * 4, "host_vs_device_result_rel_l2": err}
         del hproj, hvol

@@ -32,6 +32,9 @@ namespace lam {
 #ifndef LAM_KBOUNDS
 #define LAM_KBOUNDS __launch_bounds__(32)
 #endif
+#ifndef LAM_SHFL
+#define LAM_SHFL 1
+#endif
 #ifndef LAM_UNROLL
 #define LAM_UNROLL 1
 #endif
@@ -511,8 +514,13 @@ __global__ void LAM_KBOUNDS k_spread(SpreadArgs a) {
                   om = fmaf(om, dm2, cO[q]);
                 }
                 const float wM = fmaf(dM, oM, eM), wmine = fmaf(dm, om, em);
+#if LAM_SHFL
 #pragma unroll
                 for (int j2 = 0; j2 < W; ++j2) wm[u][j2] = __shfl_sync(0xffffffffu, wmine, slot_lane0 + j2);
+#else
+                kernel_weights<W>(a.kp, dm, wm[u]);
+                (void)wmine;
+#endif
                 vw[u] = make_float2(v.x * wM, v.y * wM);
                 ad[u] = tile_addr + (unsigned)((row0 + H) * kTP + col0 + H + j1) * 8u;
               }
