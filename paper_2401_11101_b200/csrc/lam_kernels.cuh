@@ -32,6 +32,12 @@ namespace lam {
 #ifndef LAM_KBOUNDS
 #define LAM_KBOUNDS __launch_bounds__(32)
 #endif
+#ifndef LAM_X1_MINB
+#define LAM_X1_MINB 4
+#endif
+#ifndef LAM_ROWS_MINB
+#define LAM_ROWS_MINB 1
+#endif
 #ifndef LAM_SHFL
 #define LAM_SHFL 1
 #endif
@@ -71,7 +77,7 @@ struct RowsArgs {
 };
 
 template <int LOGW, bool RAW>
-__global__ void __launch_bounds__(256) k_rows(RowsArgs a) {
+__global__ void __launch_bounds__(256, LAM_ROWS_MINB) k_rows(RowsArgs a) {
   constexpr int w = 1 << LOGW, P = fft_span(w);
   extern __shared__ float2 sm[];
   const int th = blockIdx.y, pair0 = blockIdx.x * a.nb;
@@ -601,7 +607,7 @@ struct IfftArgs {
 };
 
 template <int LOGM>
-__global__ void __launch_bounds__(256) k_ifft_x1(IfftArgs a) {
+__global__ void __launch_bounds__(256, LAM_X1_MINB) k_ifft_x1(IfftArgs a) {
   constexpr int M = 1 << LOGM, P = fft_span(M);
   extern __shared__ float2 sm[];
   const int pl = blockIdx.y, r0 = blockIdx.x * a.nb;
