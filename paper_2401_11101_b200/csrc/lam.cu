@@ -20,12 +20,6 @@
 #include "lam_kernels.cuh"
 #include "lam_forward.cuh"
 
-#ifndef LAM_X2_LNB
-#define LAM_X2_LNB 3
-#endif
-#ifndef LAM_ZTHREADS
-#define LAM_ZTHREADS 512
-#endif
 using namespace lam;
 
 namespace {
@@ -208,7 +202,7 @@ struct Launch {
   }
   static void z(dim3 g, size_t sm, cudaStream_t s, const ZArgs& a) {
     cudaFuncSetAttribute(k_zstage<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    k_zstage<L><<<g, LAM_ZTHREADS, sm, s>>>(a);
+    k_zstage<L><<<g, 512, sm, s>>>(a);
       note_launch();
   }
 };
@@ -525,7 +519,7 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   p->x1_nb = std::max(1, std::min(M, 4096 / M));
   auto tfast_lognb = [](int len, int lmax = 3) { int l = lmax; while (l > 0 && (size_t)(1 << l) * fft_tfast_pitch(len, 1 << l) * 8 > 200 * 1024) --l; return l; };
   p->cols_lcb = tfast_lognb(h);
-  p->x2_lnb = tfast_lognb(M, LAM_X2_LNB);
+  p->x2_lnb = tfast_lognb(M);
   if (n % 8) return bail(fail(p, LAM_EUNSUPPORTED, "n must be a multiple of 8"));
   if (zstage_smem(p) > 220 * 1024) return bail(fail(p, LAM_EUNSUPPORTED, "x3 stage does not fit shared memory (h = %d, sigma*nz = %d)", h, M3));
   // workspace: batch sizes from the budget

@@ -18,42 +18,13 @@
 
 namespace lam {
 
-#ifndef LAM_TILE
-#define LAM_TILE 32
-#define LAM_TP 32
-#define LAM_NU 1
-#endif
-#ifndef LAM_HALO
-#define LAM_HALO 0
-#endif
-#ifndef LAM_SEGS
-#define LAM_SEGS 32
-#endif
-#ifndef LAM_KBOUNDS
-#define LAM_KBOUNDS __launch_bounds__(32)
-#endif
-#ifndef LAM_X1_MINB
-#define LAM_X1_MINB 4
-#endif
-#ifndef LAM_ROWS_MINB
-#define LAM_ROWS_MINB 1
-#endif
-#ifndef LAM_SHFL
-#define LAM_SHFL 1
-#endif
-#ifndef LAM_UNROLL
-#define LAM_UNROLL 1
-#endif
-#ifndef LAM_QL
-#define LAM_QL 0
-#endif
-constexpr int kTile = LAM_TILE;               // gridding tile edge (fine-grid cells owned by a job)
-constexpr int kTP = LAM_TP;                 // float2 elements per storage row in shared memory (multiple of 16, >= kTile + 2W - 2)
-constexpr int kNU = LAM_NU;                  // samples a lane spreads per step (4*kNU concurrent slots per warp)
-constexpr int kSweepUnroll = LAM_UNROLL;  // unrolling of the slot sweep loop of k_spread
-constexpr bool kHalo = LAM_HALO != 0;    // storage tile with a kernel halo (no per-tap bounds tests) or without
-constexpr int kStage = 64;              // samples of one line segment parked in shared memory
-constexpr int kJobSegs = LAM_SEGS;            // target segments (theta crossings) per job
+// Tuning constants of k_spread, each chosen by same-box A/B timings on configs[2].
+constexpr int kTile = 32;         // gridding tile edge (fine-grid cells owned by a job)
+constexpr int kTP = 32;           // float2 elements per storage row in shared memory (a multiple of 16)
+constexpr int kNU = 1;            // samples a lane spreads per step (4*kNU concurrent slots per warp)
+constexpr bool kHalo = false;     // storage tile with a kernel halo (no per-tap bounds tests) or without (more warps)
+constexpr int kStage = 64;        // samples of one line segment parked in shared memory
+constexpr int kJobSegs = 32;      // target segments (theta crossings) per job
 constexpr int kJobMaxSpan = 1023;       // max theta span of one job (10 bits)
 constexpr int kMaxW = 8;
 
@@ -77,7 +48,7 @@ struct RowsArgs {
 };
 
 template <int LOGW, bool RAW>
-__global__ void __launch_bounds__(256, LAM_ROWS_MINB) k_rows(RowsArgs a) {
+__global__ void __launch_bounds__(256) k_rows(RowsArgs a) {
   constexpr int w = 1 << LOGW, P = fft_span(w);
   extern __shared__ float2 sm[];
   const int th = blockIdx.y, pair0 = blockIdx.x * a.nb;
@@ -389,7 +360,7 @@ __global__ void k_zero_tiles(SpreadArgs a) {
 // two runs of 6 contiguous cells of a half-warp sit 7..10 columns apart in rows whose pitch is a multiple of 16:
 // 12 distinct banks per 128-byte wavefront, no conflicts by construction.
 template <int W>
-__global__ void LAM_KBOUNDS k_spread(SpreadArgs a) {
+__global__ void __launch_bounds__(32) k_spread(SpreadArgs a) {
   extern __shared__ float2 tile[];
   constexpr int H = kHalo ? W - 1 : 0;               // low-side halo of the storage (0: taps are bounds-tested)
   constexpr int ROWS = kHalo ? kTile + 2 * W - 2 : kTile;
@@ -484,10 +455,8 @@ __global__ void LAM_KBOUNDS k_spread(SpreadArgs a) {
             }
             const int nseg = min(n - seg, kStage);
             // 4*kNU slots (kNU per lane) take samples Qe apart; one sweep of Qe steps covers the segment
-            // concurrent samples must be >= W cells apart along the major axis: Q_line = ceil(W / |aM|) (<= Q)
-            const int Ql = LAM_QL ? min(Q, (int)ceilf((float)W / fabsf(aM) + 1e-3f)) : Q;
-            const int Qe = max(Ql, (nseg + 4 * kNU - 1) / (4 * kNU));
-#pragma unroll kSweepUnroll
+            const int Qe = max(Q, (nseg + 4 * kNU - 1) / (4 * kNU));
+#pragma unroll 1
             for (int it = 0; it < Qe; ++it) {
               float2 acc[kNU][W];
               float wm[kNU][W];
@@ -520,13 +489,8 @@ __global__ void LAM_KBOUNDS k_spread(SpreadArgs a) {
                   om = fmaf(om, dm2, cO[q]);
                 }
                 const float wM = fmaf(dM, oM, eM), wmine = fmaf(dm, om, em);
-#if LAM_SHFL
 #pragma unroll
                 for (int j2 = 0; j2 < W; ++j2) wm[u][j2] = __shfl_sync(0xffffffffu, wmine, slot_lane0 + j2);
-#else
-                kernel_weights<W>(a.kp, dm, wm[u]);
-                (void)wmine;
-#endif
                 vw[u] = make_float2(v.x * wM, v.y * wM);
                 ad[u] = tile_addr + (unsigned)((row0 + H) * kTP + col0 + H + j1) * 8u;
               }
@@ -607,7 +571,7 @@ struct IfftArgs {
 };
 
 template <int LOGM>
-__global__ void __launch_bounds__(256, LAM_X1_MINB) k_ifft_x1(IfftArgs a) {
+__global__ void __launch_bounds__(256, 4) k_ifft_x1(IfftArgs a) {
   constexpr int M = 1 << LOGM, P = fft_span(M);
   extern __shared__ float2 sm[];
   const int pl = blockIdx.y, r0 = blockIdx.x * a.nb;
