@@ -637,7 +637,7 @@ static void launch_z(lam_plan* p, float* out, size_t zstride, int x2_0, int rows
 static lam_status init_host_path(lam_plan* p) {
   if (p->host_path_ready) return LAM_OK;
   const size_t esz = p->prm.input == LAM_INPUT_U16_RAW ? 2 : 4;
-  p->ZR = (int)std::max<size_t>(1, std::min<size_t>(p->n, (64u << 20) / ((size_t)p->nz * p->n * 4)));
+  p->ZR = (int)std::max<size_t>(1, std::min<size_t>(p->n, ((size_t)256 << 20) / ((size_t)p->nz * p->n * 4)));
   while (p->n % p->ZR) --p->ZR;
   lam_status st;
   for (int i = 0; i < 2; ++i) {
