@@ -527,10 +527,10 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   if (cudaMemGetInfo(&freeb, &totalb) != cudaSuccess) return bail(fail(p, LAM_ECUDA, "cudaMemGetInfo failed"));
   size_t budget = P.device_bytes ? P.device_bytes : (size_t)(0.9 * (double)freeb);
   const size_t gplane = (size_t)M * M * 8, tplane = (size_t)M * n * 8;
-  p->PB = P.plane_batch > 0 ? P.plane_batch : (int)std::max<size_t>(1, std::min<size_t>(p->NP, ((size_t)1 << 30) / (gplane + tplane)));
+  p->PB = P.plane_batch > 0 ? P.plane_batch : (int)std::max<size_t>(1, std::min<size_t>(p->NP, ((size_t)4 << 30) / (gplane + tplane)));
   p->PB = std::min(p->PB, p->NP);
   const size_t rproj = (size_t)h * p->WR * 8;
-  p->TC = P.theta_chunk > 0 ? P.theta_chunk : (int)std::max<size_t>(1, std::min<size_t>(n_theta, ((size_t)256 << 20) / rproj));
+  p->TC = P.theta_chunk > 0 ? P.theta_chunk : (int)std::max<size_t>(1, std::min<size_t>(n_theta, ((size_t)1 << 30) / rproj));
   p->TC = std::min(p->TC, n_theta);
   // The spectra planes S[p] die as the planes are gridded and the cropped planes A[p] are born at the same pace, so both
   // share one arena: A grows from the front, S sits right-aligned at the back; a batch of PB planes may be in flight.
