@@ -48,7 +48,7 @@ struct lam_plan {
   int M = 0, M3 = 0, W = 0, NP = 0, WR = 0, WQ = 0;
   int logw = 0, logh = 0, logM = 0, logM3 = 0;
   int PB = 1, TC = 1;  // plane batch, theta chunk
-  int rows_nb = 1, cols_lcb = 3, x1_nb = 1, x2_lnb = 3, KZ = 1;
+  int rows_nb = 1, cols_lcb = 3, x1_nb = 1, x2_lnb = 3, KZ = 1, z_lcb = 3;
   GridKernel gk;
   KerPoly kp{};
   SpreadGeom geom{};
@@ -422,7 +422,7 @@ lam_status make_tables(lam_plan* p) {
   return LAM_OK;
 }
 
-size_t zstage_smem(const lam_plan* p) { return ((size_t)(p->NP + p->KZ) * kZCb + (size_t)kZCb * fft_tfast_pitch(p->M3, kZCb)) * sizeof(float2); }
+size_t zstage_smem(const lam_plan* p, int cb) { return ((size_t)(p->NP + p->KZ) * cb + (size_t)cb * fft_tfast_pitch(p->M3, cb)) * sizeof(float2); }
 
 }  // namespace
 
@@ -521,7 +521,10 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   p->cols_lcb = tfast_lognb(h);
   p->x2_lnb = tfast_lognb(M);
   if (n % 8) return bail(fail(p, LAM_EUNSUPPORTED, "n must be a multiple of 8"));
-  if (zstage_smem(p) > 220 * 1024) return bail(fail(p, LAM_EUNSUPPORTED, "x3 stage does not fit shared memory (h = %d, sigma*nz = %d)", h, M3));
+  // x3 stage: 8 columns per block, fewer when that would leave one block per SM (>= 2 blocks of <= 100 KB)
+  p->z_lcb = 3;
+  while (p->z_lcb > 1 && zstage_smem(p, 1 << p->z_lcb) > 100 * 1024) --p->z_lcb;
+  if (zstage_smem(p, 1 << p->z_lcb) > 220 * 1024) return bail(fail(p, LAM_EUNSUPPORTED, "x3 stage does not fit shared memory (h = %d, sigma*nz = %d)", h, M3));
   // workspace: batch sizes from the budget
   size_t freeb = 0, totalb = 0;
   if (cudaMemGetInfo(&freeb, &totalb) != cudaSuccess) return bail(fail(p, LAM_ECUDA, "cudaMemGetInfo failed"));
@@ -629,8 +632,8 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
 static void launch_z(lam_plan* p, float* out, size_t zstride, int x2_0, int rows, int out_x2_0, cudaStream_t s) {
   StageScope sc(p, 3, s);
   ZArgs za{p->d_A, out, zstride, p->d_tw_M3, p->d_ztab, p->d_zlo, p->d_zcnt, p->d_zlast, p->d_dx, p->d_dz,
-           p->n, p->nz, p->NP, p->KZ, x2_0, out_x2_0};
-  DISPATCH_LOG(p->logM3, z(dim3(p->n / kZCb, rows), zstage_smem(p), s, za));
+           p->n, p->nz, p->NP, p->KZ, p->z_lcb, x2_0, out_x2_0};
+  DISPATCH_LOG(p->logM3, z(dim3(p->n >> p->z_lcb, rows), zstage_smem(p, 1 << p->z_lcb), s, za));
   p->launches += 1;
 }
 

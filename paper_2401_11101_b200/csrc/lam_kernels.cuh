@@ -609,7 +609,7 @@ __global__ void __launch_bounds__(512) k_ifft_x2(IfftArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// x3 stage, one block per (x2, group of 8 x1): xi3 = k_v cos(phi)/h depends on k_v only (Eq. 6), so the planes
+// x3 stage, one block per (x2, group of 2..8 x1): xi3 = k_v cos(phi)/h depends on k_v only (Eq. 6), so the planes
 // A[p] are samples of a 1-D unequally spaced spectrum along x3 for every (x1, x2):
 //   Gz[m3] = sum_p A[p] kap(t3(p) - m3),  t3 = M3 k_v cos(phi)/h;   vol[x3] = Re sum_m3 Gz[m3] e^{2 pi i x3 m3/M3}
 //   divided by kaphat(x1/M) kaphat(x2/M) kaphat(x3/M3)  (PAPER.md:136 step 1, reversed per PAPER.md:140).
@@ -630,36 +630,37 @@ struct ZArgs {
   const float* zlast;    // [M3]
   const float* dx;       // [n]  1/kaphat(x/M)
   const float* dz;       // [nz] 1/kaphat(x3/M3)
-  int n, nz, np, KZ;
+  int n, nz, np, KZ, lcb;  // 1 << lcb columns per block
   int x2_0;              // first x2 row of this launch
   int vol_x2_0;          // x2 index held by row 0 of the output buffer
 };
 
 template <int LOGM3>
 __global__ void __launch_bounds__(512) k_zstage(ZArgs a) {
-  constexpr int M3 = 1 << LOGM3, P = fft_tfast_pitch(M3, kZCb);
+  constexpr int M3 = 1 << LOGM3;
+  const int zlog = a.lcb, zcb = 1 << a.lcb, P = fft_tfast_pitch(M3, zcb);  // columns per block
   extern __shared__ float2 sm[];
   float2* Gz = sm;                                // [8][P]
-  float2* Ain = sm + kZCb * P;                    // [np + KZ][8], the KZ extra planes are zero
-  const int ix2 = a.x2_0 + blockIdx.y, c0 = blockIdx.x * kZCb;
+  float2* Ain = sm + zcb * P;                    // [np + KZ][zcb], the KZ extra planes are zero
+  const int ix2 = a.x2_0 + blockIdx.y, c0 = blockIdx.x * zcb;
   const size_t nn = (size_t)a.n * a.n;
   const float2* Ab = a.A + (size_t)ix2 * a.n + c0;
-  for (int idx = threadIdx.x; idx < (a.np + a.KZ) * kZCb; idx += blockDim.x) {
-    int p = idx >> kZLog, c = idx & (kZCb - 1);
+  for (int idx = threadIdx.x; idx < (a.np + a.KZ) * zcb; idx += blockDim.x) {
+    int p = idx >> zlog, c = idx & (zcb - 1);
     Ain[idx] = p < a.np ? Ab[(size_t)p * nn + c] : make_float2(0.f, 0.f);
   }
   __syncthreads();
-  const int KZ = a.KZ, last = (a.np - 1) * kZCb;
+  const int KZ = a.KZ, last = (a.np - 1) * zcb;
   auto ld = [&](int t, int i) -> float2 {
     const float* wt = a.ztab + (size_t)i * KZ;
-    const float2* ap = Ain + __ldg(&a.zlo[i]) * kZCb + t;
+    const float2* ap = Ain + __ldg(&a.zlo[i]) * zcb + t;
     float wl = __ldg(&a.zlast[i]);
     float2 v = Ain[last + t];
     float2 acc = make_float2(v.x * wl, v.y * wl);
     const int cnt = __ldg(&a.zcnt[i]);
     for (int s = 0; s < cnt; ++s) {
       float wv = __ldg(&wt[s]);
-      float2 x = ap[s * kZCb];
+      float2 x = ap[s * zcb];
       acc.x = fmaf(x.x, wv, acc.x);
       acc.y = fmaf(x.y, wv, acc.y);
     }
@@ -673,7 +674,7 @@ __global__ void __launch_bounds__(512) k_zstage(ZArgs a) {
     if (k >= hz && k < M3 - hz) return;
     vb[(size_t)ix3 * a.zstride + t] = v.x * a.dz[ix3] * dx2 * a.dx[c0 + t];
   };
-  block_fft<LOGM3, +1, true, true>(Gz, kZCb, kZLog, P, a.tw, ld, st);
+  block_fft<LOGM3, +1, true, true>(Gz, zcb, zlog, P, a.tw, ld, st);
 }
 
 }  // namespace lam
