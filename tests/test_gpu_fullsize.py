@@ -86,8 +86,11 @@ def test_config4_out_of_core_host_buffers():
     need_host = cfg.ntheta * cfg.h * cfg.w * 2 + cfg.voxels * 4
     if free < 150e9 or psutil.virtual_memory().available < need_host + 20e9:
         pytest.skip("configs[4] needs ~145 GB of device memory and ~135 GB of host memory")
-    proj, sel, proj_sel, dark, flat = sparse_scan(cfg, "cpu")
-    vol = torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, pin_memory=True)
+    try:
+        proj, sel, proj_sel, dark, flat = sparse_scan(cfg, "cpu")
+        vol = torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, pin_memory=True)
+    except RuntimeError as e:  # the host refuses to pin ~115 GB
+        pytest.skip(f"cannot allocate the pinned host buffers of configs[4]: {e}")
     plan = lam.Plan(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
                     input="u16")
     plan.set_darkflat(dark.cuda(), flat.cuda())
