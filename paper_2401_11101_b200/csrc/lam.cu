@@ -63,6 +63,8 @@ struct lam_plan {
   int *d_zlo = nullptr, *d_zcnt = nullptr;
   uint2* d_jobs = nullptr;
   std::vector<long long> job_off;  // [NP+1] first job of each plane
+  unsigned* d_multi = nullptr;     // tiles written by several jobs, plane-major
+  std::vector<long long> multi_off;  // [NP+1]
   // workspace
   float2 *d_R = nullptr, *d_S = nullptr, *d_G = nullptr, *d_T = nullptr, *d_A = nullptr;  // d_S, d_A live inside d_arena
   float2* d_arena = nullptr;
@@ -247,7 +249,7 @@ struct StageScope {
 
 void free_all(lam_plan* p) {
   void* ptrs[] = {p->d_cs,    p->d_Pu,  p->d_Pv,  p->d_PuNone, p->d_tw_w, p->d_tw_h,   p->d_tw_M, p->d_tw_M3,
-                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_zcnt, p->d_df, p->d_wz, p->d_bz,
+                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_zcnt, p->d_df, p->d_wz, p->d_bz, p->d_multi,
                   p->d_R,     p->d_arena, p->d_G, p->d_T};
   for (void* q : ptrs)
     if (q) cudaFree(q);
@@ -306,6 +308,17 @@ lam_status build_jobs(lam_plan* p) {
     }
     p->job_off[p->NP] = tot;
     st = dalloc(p, &p->d_jobs, (size_t)tot);
+    // tiles with several jobs: zeroed before each spreading, then merged with atomic adds
+    std::vector<unsigned> multi;
+    p->multi_off.assign(p->NP + 1, 0);
+    const int nt = p->geom.nt;
+    for (int pl = 0; pl < p->NP; ++pl) {
+      p->multi_off[pl] = (long long)multi.size();
+      for (int t = 0; t < ntiles; ++t)
+        if (counts[(size_t)pl * ntiles + t] > 1) multi.push_back((unsigned)pl << 18 | (unsigned)(t / nt) << 9 | (unsigned)(t % nt));
+    }
+    p->multi_off[p->NP] = (long long)multi.size();
+    if (st == LAM_OK) st = upload(p, &p->d_multi, multi);
   }
   std::vector<unsigned> offs(scratch);
   for (int p0 = 0; p0 < p->NP && st == LAM_OK; p0 += chunk) {
@@ -603,10 +616,11 @@ static void launch_s1(lam_plan* p, const void* chunk, int th0, int nth, cudaStre
 
 // S2 + S3 (x1, x2) for planes [p0, p0 + np)
 static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
-  SpreadArgs sa{p->geom, p->kp, p->d_jobs + p->job_off[p0], p->job_off[p0 + np] - p->job_off[p0], p->d_S, p->WQ, p->d_G, p0};
+  SpreadArgs sa{p->geom, p->kp, p->d_jobs + p->job_off[p0], p->job_off[p0 + np] - p->job_off[p0], p->d_S, p->WQ, p->d_G, p0,
+                p->d_multi + p->multi_off[p0], p->multi_off[p0 + np] - p->multi_off[p0]};
   {
     StageScope sc(p, 1, s);
-    k_zero_tiles<<<(unsigned)((sa.njobs + 7) / 8), 256, 0, s>>>(sa);
+    if (sa.nmulti > 0) k_zero_tiles<<<(unsigned)((sa.nmulti + 7) / 8), 256, 0, s>>>(sa);
       note_launch();
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;

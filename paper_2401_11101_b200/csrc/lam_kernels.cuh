@@ -332,26 +332,28 @@ struct SpreadArgs {
   int WQ;
   float2* G;           // [planes in batch][M][M]
   int p0;              // first plane of the batch
+  const unsigned* multi;  // tiles of the batch's planes that several jobs write (k_zero_tiles)
+  long long nmulti;
 };
 
-// zero the tiles that receive atomic adds from several jobs (one warp per job word; only the first job of a tile acts)
+// zero the tiles that receive atomic adds from several jobs: one warp per entry of the plan's list of such tiles
+// (entry = plane << 18 | ty << 9 | tx, built once from the job counts)
 __global__ void k_zero_tiles(SpreadArgs a) {
   const int lane = threadIdx.x & 31;
   long long j = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (j >= a.njobs) return;
-  uint2 jb = a.jobs[j];
-  if (!((jb.y >> 16) & kJobFirstMulti)) return;
+  if (j >= a.nmulti) return;
+  const unsigned e = a.multi[j];
   const int M = a.g.M;
-  int tx = jb.x & 0x1ff, ty = (jb.x >> 9) & 0x1ff, p = (jb.y >> 18) & 0x1fff;
+  int tx = e & 0x1ff, ty = (e >> 9) & 0x1ff, p = e >> 18;
   float2* Gp = a.G + (size_t)(p - a.p0) * M * M;
   const int x0 = tx * kTile, y0 = ty * kTile;
   for (int r = 0; r < kTile && y0 + r < M; ++r)
     for (int c = lane; c < kTile && x0 + c < M; c += 32) Gp[(size_t)(y0 + r) * M + x0 + c] = make_float2(0.f, 0.f);
 }
 
-// Spreading of one job.  The warp owns a private storage tile [kTile + 2W - 2][kTP] in shared memory that covers the
-// owned cells plus the kernel halo, so every tap of every visited sample lands inside it and needs no bounds test;
-// a sample is visited iff its W x W footprint meets the owned kTile x kTile cells.
+// Spreading of one job.  The warp owns a private storage tile [kTile][kTP] in shared memory; a sample is visited
+// iff its W x W footprint meets the kTile x kTile cells, and every tap is bounds-tested against the tile (the variant
+// with a kernel halo around the tile and no tests, kHalo, halves the resident warps and is slower).
 //
 // Lane roles: half-warp h holds two slots of W lanes; lane j of a slot owns tap column j of the slot's current
 // sample (along the MAJOR axis: x for x-dominant lines, y for y-dominant lines, whose jobs work on the transposed
