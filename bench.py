@@ -278,6 +278,9 @@ def run_ours(args):
             if int(row["config"]) == args.config and row["stage"] == names[dom]:
                 roof["traffic"] = float(row["dram_bytes_per_launch"])
                 roof["traffic_note"] = row["source"]
+                if row.get("issue_active_pct"):  # what binds the kernel under ncu: issue slots and the shared-memory pipe
+                    roof["ncu_issue_active_pct"] = float(row["issue_active_pct"])
+                    roof["ncu_l1tex_throughput_pct"] = float(row["l1tex_throughput_pct"])
     except Exception:
         pass
     roof["stages"] = stages
