@@ -18,6 +18,7 @@
 
 #include "../../include/lam.h"
 #include "lam_kernels.cuh"
+#include "lam_spread.cuh"
 #include "lam_forward.cuh"
 
 using namespace lam;
@@ -61,10 +62,11 @@ struct lam_plan {
   float* d_wz = nullptr;  // [NP][W] x3 tap weights per plane (lam_forward)
   int* d_bz = nullptr;    // [NP] first x3 tap per plane
   int *d_zlo = nullptr, *d_zcnt = nullptr;
-  uint2* d_jobs = nullptr;
-  std::vector<long long> job_off;  // [NP+1] first job of each plane
-  unsigned* d_multi = nullptr;     // tiles written by several jobs, plane-major
-  std::vector<long long> multi_off;  // [NP+1]
+  Job* d_jobs = nullptr;
+  std::vector<long long> job_off;  // [batches+1] first job of each plane batch (jobs of a batch: heaviest tiles first)
+  unsigned* d_multi = nullptr;     // tiles written by several jobs, batch-major
+  std::vector<long long> multi_off;  // [batches+1]
+  double plan_ms = 0;              // wall time of lam_create
   // workspace
   float2 *d_R = nullptr, *d_S = nullptr, *d_G = nullptr, *d_T = nullptr, *d_A = nullptr;  // d_S, d_A live inside d_arena
   float2* d_arena = nullptr;
@@ -271,70 +273,80 @@ void free_all(lam_plan* p) {
 }
 
 // ---- work lists of the (xi1, xi2) gridding: geometry only, built once ---------------------------------------------
+// Two device passes (count, fill) with the host in between: the jobs of one plane batch (= one k_spread launch) are laid
+// out heaviest tile first, so that the few tiles around the xi3 axis that every theta crosses start early.
 lam_status build_jobs(lam_plan* p) {
-  const int ntiles = p->geom.nt * p->geom.nt;
-  const int chunk = std::max(1, std::min(p->NP, (1 << 23) / ntiles));
-  unsigned *d_count = nullptr, *d_off = nullptr;
-  size_t scratch = (size_t)chunk * ntiles;
-  if (cudaMalloc(&d_count, scratch * 4) != cudaSuccess || cudaMalloc(&d_off, scratch * 4) != cudaSuccess) {
+  const int ntiles = p->geom.nt * p->geom.nt, NP = p->NP, PB = p->PB;
+  const int chunk = std::max(1, std::min(NP, (1 << 22) / ntiles));
+  unsigned *d_count = nullptr, *d_lines = nullptr, *d_off = nullptr;
+  const size_t scratch = (size_t)chunk * ntiles;
+  if (cudaMalloc(&d_count, scratch * 4) != cudaSuccess || cudaMalloc(&d_lines, scratch * 4) != cudaSuccess ||
+      cudaMalloc(&d_off, scratch * 4) != cudaSuccess) {
     cudaGetLastError();
     if (d_count) cudaFree(d_count);
-    return fail(p, LAM_ENOMEM_DEVICE, "work-list scratch of %zu bytes does not fit", scratch * 8);
+    if (d_lines) cudaFree(d_lines);
+    return fail(p, LAM_ENOMEM_DEVICE, "work-list scratch of %zu bytes does not fit", scratch * 12);
   }
-  std::vector<unsigned> counts((size_t)p->NP * ntiles);
+  std::vector<unsigned> counts((size_t)NP * ntiles), lines((size_t)NP * ntiles), offs((size_t)NP * ntiles);
   lam_status st = LAM_OK;
-  auto launch = [&](int p0, int np, bool fill, uint2* jobs) {
-    JobsArgs a{p->geom, p0, np, d_count, d_off, jobs};
-    long long total = (long long)np * ntiles;
-    unsigned blocks = (unsigned)((total + 127) / 128);
+  auto launch = [&](int p0, int np, bool fill) {
+    JobsArgs a{p->geom, p0, np, d_count, d_lines, d_off, p->d_jobs};
+    const long long total = (long long)np * ntiles;
+    const unsigned blocks = (unsigned)((total + 63) / 64);
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;
-      if (fill) k_jobs<W, true><<<blocks, 128>>>(a);
-      else k_jobs<W, false><<<blocks, 128>>>(a);
+      if (fill) k_jobs<W, true><<<blocks, 64>>>(a);
+      else k_jobs<W, false><<<blocks, 64>>>(a);
     });
   };
-  for (int p0 = 0; p0 < p->NP && st == LAM_OK; p0 += chunk) {
-    int np = std::min(chunk, p->NP - p0);
-    launch(p0, np, false, nullptr);
+  for (int p0 = 0; p0 < NP && st == LAM_OK; p0 += chunk) {
+    const int np = std::min(chunk, NP - p0);
+    launch(p0, np, false);
     cudaError_t e = cudaMemcpy(counts.data() + (size_t)p0 * ntiles, d_count, (size_t)np * ntiles * 4, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(lines.data() + (size_t)p0 * ntiles, d_lines, (size_t)np * ntiles * 4, cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) st = fail(p, LAM_ECUDA, "work-list count pass: %s", cudaGetErrorString(e));
   }
   if (st == LAM_OK) {
-    p->job_off.assign(p->NP + 1, 0);
-    long long tot = 0;
-    for (int pl = 0; pl < p->NP; ++pl) {
-      p->job_off[pl] = tot;
-      for (int t = 0; t < ntiles; ++t) tot += counts[(size_t)pl * ntiles + t];
-    }
-    p->job_off[p->NP] = tot;
-    st = dalloc(p, &p->d_jobs, (size_t)tot);
-    // tiles with several jobs: zeroed before each spreading, then merged with atomic adds
+    const int nb = (NP + PB - 1) / PB;
+    p->job_off.assign(nb + 1, 0);
+    p->multi_off.assign(nb + 1, 0);
     std::vector<unsigned> multi;
-    p->multi_off.assign(p->NP + 1, 0);
+    std::vector<unsigned> order;
+    long long tot = 0;
     const int nt = p->geom.nt;
-    for (int pl = 0; pl < p->NP; ++pl) {
-      p->multi_off[pl] = (long long)multi.size();
-      for (int t = 0; t < ntiles; ++t)
-        if (counts[(size_t)pl * ntiles + t] > 1) multi.push_back((unsigned)pl << 18 | (unsigned)(t / nt) << 9 | (unsigned)(t % nt));
+    for (int b = 0; b < nb; ++b) {
+      const size_t i0 = (size_t)b * PB * ntiles, i1 = (size_t)std::min(NP, (b + 1) * PB) * ntiles;
+      p->job_off[b] = tot;
+      p->multi_off[b] = (long long)multi.size();
+      order.resize(i1 - i0);
+      for (size_t i = 0; i < order.size(); ++i) order[i] = (unsigned)i;
+      std::stable_sort(order.begin(), order.end(), [&](unsigned x, unsigned y) { return lines[i0 + x] > lines[i0 + y]; });
+      for (unsigned o : order) {
+        const size_t i = i0 + o;
+        offs[i] = (unsigned)tot;
+        tot += counts[i];
+        if (counts[i] > 1) {
+          const unsigned pl = (unsigned)(i / ntiles), t = (unsigned)(i % ntiles);
+          multi.push_back(pl << 16 | (unsigned)(t / nt) << 8 | (unsigned)(t % nt));
+        }
+      }
     }
-    p->multi_off[p->NP] = (long long)multi.size();
+    p->job_off[nb] = tot;
+    p->multi_off[nb] = (long long)multi.size();
+    if (tot > 0xffffffffLL) st = fail(p, LAM_EUNSUPPORTED, "more than 2^32 gridding jobs");
+    if (st == LAM_OK) st = dalloc(p, &p->d_jobs, (size_t)tot);
     if (st == LAM_OK) st = upload(p, &p->d_multi, multi);
   }
-  std::vector<unsigned> offs(scratch);
-  for (int p0 = 0; p0 < p->NP && st == LAM_OK; p0 += chunk) {
-    int np = std::min(chunk, p->NP - p0);
-    unsigned run = 0;
-    for (size_t i = 0; i < (size_t)np * ntiles; ++i) {
-      offs[i] = run;
-      run += counts[(size_t)p0 * ntiles + i];
-    }
-    cudaMemcpy(d_off, offs.data(), (size_t)np * ntiles * 4, cudaMemcpyHostToDevice);
+  for (int p0 = 0; p0 < NP && st == LAM_OK; p0 += chunk) {
+    const int np = std::min(chunk, NP - p0);
+    cudaMemcpy(d_off, offs.data() + (size_t)p0 * ntiles, (size_t)np * ntiles * 4, cudaMemcpyHostToDevice);
     cudaMemcpy(d_count, counts.data() + (size_t)p0 * ntiles, (size_t)np * ntiles * 4, cudaMemcpyHostToDevice);
-    launch(p0, np, true, p->d_jobs + p->job_off[p0]);
+    launch(p0, np, true);
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) st = fail(p, LAM_ECUDA, "work-list fill pass: %s", cudaGetErrorString(e));
   }
   cudaFree(d_count);
+  cudaFree(d_lines);
   cudaFree(d_off);
   return st;
 }
@@ -427,11 +439,10 @@ lam_status make_tables(lam_plan* p) {
   g.rho_unit = (double)M * std::sin(p->phi) / h;
   g.a1 = (float)M / (float)w;
   g.M = M;
-  g.nt = (M + kTile - 1) / kTile;
+  g.nt = M / kTS;
   g.ntheta = p->ntheta;
   g.w = w;
   g.hh = h / 2;
-  g.kstride = std::max(1, (int)std::ceil(1.0002 * std::sqrt(2.0) * W * w / M));  // samples between concurrently spread slots
   return LAM_OK;
 }
 
@@ -499,8 +510,8 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   const int lo = 1 << kLogMin, hi = 1 << kLogMax;
   if (w < lo || w > hi || h < lo || h > hi || M < 64 || M > hi || M3 < lo || M3 > hi)
     return fail(nullptr, LAM_EUNSUPPORTED, "w, h, sigma*nz must be in [32, 8192] and sigma*n in [64, 8192]");
-  if (h / 2 + 1 > 0x1fff || (M + kTile - 1) / kTile > 0x1ff || n_theta > 0x3fff)
-    return fail(nullptr, LAM_EUNSUPPORTED, "h <= 16382, sigma*n <= 16352 and n_theta <= 16383 in this build");
+  if (h / 2 + 1 > 0x1fff || M / kTS > 0x100 || n_theta > 0x3fff)
+    return fail(nullptr, LAM_EUNSUPPORTED, "h <= 16382, sigma*n <= 16384 and n_theta <= 16383 in this build");
   if (M3 < 2 * P.width || M < 2 * P.width) return fail(nullptr, LAM_EINVAL, "grid smaller than the kernel footprint");
 
   int ndev = 0;
@@ -614,19 +625,23 @@ static void launch_s1(lam_plan* p, const void* chunk, int th0, int nth, cudaStre
   p->launches += 2;
 }
 
-// S2 + S3 (x1, x2) for planes [p0, p0 + np)
+// S2 + S3 (x1, x2) for planes [p0, p0 + np): p0 is a multiple of the plane batch
 static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
-  SpreadArgs sa{p->geom, p->kp, p->d_jobs + p->job_off[p0], p->job_off[p0 + np] - p->job_off[p0], p->d_S, p->WQ, p->d_G, p0,
-                p->d_multi + p->multi_off[p0], p->multi_off[p0 + np] - p->multi_off[p0]};
+  const int b = p0 / p->PB;
+  SpreadArgs sa{p->geom, p->kp, p->d_jobs + p->job_off[b], p->job_off[b + 1] - p->job_off[b], p->d_S, p->WQ, p->d_G, p0,
+                p->d_multi + p->multi_off[b], p->multi_off[b + 1] - p->multi_off[b]};
   {
     StageScope sc(p, 1, s);
-    if (sa.nmulti > 0) k_zero_tiles<<<(unsigned)((sa.nmulti + 7) / 8), 256, 0, s>>>(sa);
+    if (sa.nmulti > 0) {
+      k_zero_tiles<<<(unsigned)((sa.nmulti + 7) / 8), 256, 0, s>>>(sa);
       note_launch();
+      p->launches += 1;
+    }
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;
-      size_t sm = ((size_t)(kHalo ? kTile + 2 * W - 2 : kTile) * kTP + 2 * kStage) * sizeof(float2);
+      const size_t sm = (size_t)kTS * kTS * sizeof(float2) + (size_t)kSW * 32 * sizeof(LineParams);
       cudaFuncSetAttribute(k_spread<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-      k_spread<W><<<(unsigned)sa.njobs, 32, sm, s>>>(sa);
+      k_spread<W><<<(unsigned)sa.njobs, 32 * kSW, sm, s>>>(sa);
       note_launch();
     });
   }
@@ -639,7 +654,7 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
     DISPATCH_LOG(p->logM, x2(dim3(p->n / nb2, np), (size_t)nb2 * p->M >= 16384 ? 512 : 256,
                              (size_t)nb2 * fft_tfast_pitch(p->M, nb2) * sizeof(float2), s, a2));
   }
-  p->launches += 4;
+  p->launches += 3;
 }
 
 // x3 stage for x2 rows [x2_0, x2_0 + rows); out holds x2 row `out_x2_0` in its first row, z-stride `zstride` floats

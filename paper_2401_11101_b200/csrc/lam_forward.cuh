@@ -15,6 +15,7 @@
 // weights stay.
 #pragma once
 #include "lam_kernels.cuh"
+#include "lam_spread.cuh"
 
 namespace lam {
 

@@ -3,8 +3,7 @@
 // Stage map (S-numbers are SURVEY.md §8(a) rows):
 //   k_rows     S0+S1  -log prep, row FFT along u of two real rows per complex transform, filter H[k_u] (Eq. 3)
 //   k_cols     S1     column FFT along v, Hermitian fold onto the k_v >= 0 planes, centring phases
-//   k_jobs_*   S2     work-list builder: which (tile, theta-range) pairs of a k_v plane hold samples (geometry only)
-//   k_spread   S2     gridding in (xi1, xi2): width-W kernel scatter of every sample of Eq. 6 onto its plane
+//   k_jobs, k_spread  S2  gridding in (xi1, xi2): lam_spread.cuh
 //   k_ifft_x1  S3     inverse FFT along xi1 -> x1, cropped to the n central outputs
 //   k_ifft_x2  S3     inverse FFT along xi2 -> x2, cropped
 //   k_zstage   S2+S3+S4  gridding in xi3 (depends on k_v only, Eq. 6), inverse FFT to x3, crop, real part,
@@ -17,16 +16,6 @@
 #include "lam_math.h"
 
 namespace lam {
-
-// Tuning constants of k_spread, each chosen by same-box A/B timings on configs[2].
-constexpr int kTile = 32;         // gridding tile edge (fine-grid cells owned by a job)
-constexpr int kTP = 32;           // float2 elements per storage row in shared memory (a multiple of 16)
-constexpr int kNU = 1;            // samples a lane spreads per step (4*kNU concurrent slots per warp)
-constexpr bool kHalo = false;     // storage tile with a kernel halo (no per-tap bounds tests) or without (more warps)
-constexpr int kStage = 64;        // samples of one line segment parked in shared memory
-constexpr int kJobSegs = 32;      // target segments (theta crossings) per job
-constexpr int kJobMaxSpan = 1023;       // max theta span of one job (10 bits)
-constexpr int kMaxW = 8;
 
 // (dark, flat) -> (dark, 1 / max(flat - dark, 1)): the per-pixel constants of the -log prep (reading Q12)
 __global__ void k_darkflat(const float* dark, const float* flat, float2* df, size_t cnt) {
@@ -127,438 +116,6 @@ __global__ void __launch_bounds__(512) k_cols(ColsArgs a) {
     emit(p, c);
   }
   if (threadIdx.x < kColsCb) emit(h / 2, threadIdx.x);
-}
-
-// ---------------------------------------------------------------------------------------------------------------
-// S2: gridding in (xi1, xi2).  Plane p (k_v fixed): sample (theta, k_u) sits at fine-grid position
-//   t = a1 k_u (cos t, sin t) + rho (sin t, -cos t),  a1 = M/w,  rho = M k_v sin(phi)/h      (Eq. 6 times M)
-// i.e. on a straight line per theta, tangent to the circle of radius rho.  The plane is cut into 32x32 tiles; a
-// job = (tile, theta-range); a warp owns a private shared-memory tile, walks the theta-range, clips every line
-// against the tile (+ kernel halo, + periodic images, reading Q7), and lets lane i deposit sample k_a + i.
-// ---------------------------------------------------------------------------------------------------------------
-struct SpreadGeom {
-  const double2* cs;   // [ntheta] (cos, sin) in double
-  double rho_unit;     // M sin(phi) / h
-  float a1;            // M / w
-  int M, nt, ntheta, w, hh /* h/2 */, kstride;
-};
-
-struct KerPoly {
-  float E[kMaxW / 2][kPolyHalf];
-  float O[kMaxW / 2][kPolyHalf];
-};
-
-// job word layout: x = tx[0:9) ty[9:18) th0[18:32);  y = nth[0:10) mx[10:13) my[13:16) flags[16:18) p[18:31) ydom[31]
-constexpr unsigned kJobExclusive = 1u, kJobFirstMulti = 2u;
-
-__device__ __forceinline__ uint2 job_pack(int tx, int ty, int th0, int nth, int mx, int my, unsigned fl, int p, int ydom) {
-  return make_uint2((unsigned)tx | ((unsigned)ty << 9) | ((unsigned)th0 << 18),
-                    (unsigned)nth | ((unsigned)mx << 10) | ((unsigned)my << 13) | (fl << 16) | ((unsigned)p << 18) |
-                        ((unsigned)ydom << 31));
-}
-
-// ku range [ka, kb] of the samples of one line whose kernel footprint can reach the tile.
-// (ox, oy): line origin relative to the tile's first cell; the sample k sits at (ox, oy) + a1 k (c, s).
-// Footprint test is conservative (margin 0.02 cells >> fp32 error of ox, oy); exact clipping is per tap.
-template <int W>
-__device__ __forceinline__ void clip_line(float ox, float oy, float c, float s, float a1, int hw, int& ka, int& kb) {
-  const float xl = -0.5f * W - 0.02f, xh = (float)(kTile - 1) + 0.5f * W + 0.02f;
-  float lo = -a1 * hw, hi = a1 * hw;
-  bool empty = false;
-  if (fabsf(c) > 1e-6f) {
-    float r = 1.0f / c, u0 = (xl - ox) * r, u1 = (xh - ox) * r;
-    lo = fmaxf(lo, fminf(u0, u1));
-    hi = fminf(hi, fmaxf(u0, u1));
-  } else if (ox < xl || ox > xh) empty = true;
-  if (fabsf(s) > 1e-6f) {
-    float r = 1.0f / s, u0 = (xl - oy) * r, u1 = (xh - oy) * r;
-    lo = fmaxf(lo, fminf(u0, u1));
-    hi = fminf(hi, fmaxf(u0, u1));
-  } else if (oy < xl || oy > xh) empty = true;
-  float ia = 1.0f / a1;
-  ka = max(-hw, (int)ceilf(lo * ia - 1e-3f));
-  kb = min(hw, (int)floorf(hi * ia + 1e-3f));
-  if (empty) { ka = 1; kb = 0; }
-}
-
-// which periodic images (shifts of -M, 0, +M per axis) of the sample cloud can reach the tile: bit sx+1 / sy+1
-__device__ __forceinline__ void image_candidates(const SpreadGeom& g, double rho, int mx0, int my0, int W, int& candx,
-                                                 int& candy) {
-  float rmax = sqrtf((float)(0.25 * (double)g.M * g.M + rho * rho)) + 0.5f * W + 1.0f;
-  candx = 0;
-  candy = 0;
-  for (int s = -1; s <= 1; ++s) {
-    // the image shifted by s*M covers [s*M - rmax, s*M + rmax]; the tile covers [m0, m0 + 31]
-    float lo = s * (float)g.M - rmax, hi = s * (float)g.M + rmax;
-    if (hi >= mx0 && lo <= mx0 + kTile - 1) candx |= 1 << (s + 1);
-    if (hi >= my0 && lo <= my0 + kTile - 1) candy |= 1 << (s + 1);
-  }
-}
-
-struct JobsArgs {
-  SpreadGeom g;
-  int p0, np;            // planes [p0, p0+np)
-  unsigned* count;       // [np][nt*nt]
-  const unsigned* off;   // [np][nt*nt] exclusive offsets within the chunk's job array (fill pass)
-  uint2* jobs;           // chunk job array (fill pass)
-};
-
-// FILL = false: count jobs per tile; FILL = true: write them.  One thread per (plane, tile).
-template <int W, bool FILL>
-__global__ void k_jobs(JobsArgs a) {
-  const SpreadGeom& g = a.g;
-  const int ntiles = g.nt * g.nt;
-  long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gid >= (long long)a.np * ntiles) return;
-  const int pl = (int)(gid / ntiles), tile = (int)(gid - (long long)pl * ntiles);
-  const int p = a.p0 + pl, ty = tile / g.nt, tx = tile - ty * g.nt;
-  const int kv = p == g.hh ? -g.hh : p;
-  const double rho = g.rho_unit * kv;
-  const int mx0 = tx * kTile - g.M / 2, my0 = ty * kTile - g.M / 2;
-  int candx, candy;
-  image_candidates(g, rho, mx0, my0, W, candx, candy);
-  // pass A: which images are ever hit (so that all jobs of the tile carry the same masks)
-  int usex = 0, usey = 0;
-  for (int th = 0; th < g.ntheta; ++th) {
-    double2 cs = g.cs[th];
-    float c = (float)cs.x, s = (float)cs.y;
-    for (int sy = -1; sy <= 1; ++sy) {
-      if (!(candy >> (sy + 1) & 1)) continue;
-      float oy = (float)(-rho * cs.x - my0 + (double)sy * g.M);
-      for (int sx = -1; sx <= 1; ++sx) {
-        if (!(candx >> (sx + 1) & 1)) continue;
-        float ox = (float)(rho * cs.y - mx0 + (double)sx * g.M);
-        int ka, kb;
-        clip_line<W>(ox, oy, c, s, g.a1, g.w / 2, ka, kb);
-        if (ka <= kb) { usex |= 1 << (sx + 1); usey |= 1 << (sy + 1); }
-      }
-    }
-  }
-  // pass B: emit jobs; a job holds lines of one orientation only (|cos| >= |sin|: x-dominant, else y-dominant)
-  unsigned njobs = 0;
-  int start = -1, last = -1, cnt = 0, ori = 0;
-  uint2* out = FILL ? a.jobs + a.off[gid] : nullptr;
-  const unsigned total = FILL ? a.count[gid] : 0;
-  auto emit = [&](int t0, int t1) {
-    if (FILL) {
-      unsigned fl = total == 1 ? kJobExclusive : (njobs == 0 ? kJobFirstMulti : 0u);
-      out[njobs] = job_pack(tx, ty, t0, t1 - t0, usex, usey, fl, p, ori);
-    }
-    ++njobs;
-  };
-  if (usex && usey) {
-    for (int th = 0; th < g.ntheta; ++th) {
-      double2 cs = g.cs[th];
-      float c = (float)cs.x, s = (float)cs.y;
-      const int o = fabsf(c) >= fabsf(s) ? 0 : 1;
-      bool hit = false;
-      for (int sy = -1; sy <= 1 && !hit; ++sy) {
-        if (!(usey >> (sy + 1) & 1)) continue;
-        float oy = (float)(-rho * cs.x - my0 + (double)sy * g.M);
-        for (int sx = -1; sx <= 1 && !hit; ++sx) {
-          if (!(usex >> (sx + 1) & 1)) continue;
-          float ox = (float)(rho * cs.y - mx0 + (double)sx * g.M);
-          int ka, kb;
-          clip_line<W>(ox, oy, c, s, g.a1, g.w / 2, ka, kb);
-          hit = ka <= kb;
-        }
-      }
-      if (start >= 0 && (o != ori || (!hit && th - last > 32))) {
-        emit(start, last + 1);
-        start = -1;
-        cnt = 0;
-      }
-      if (hit) {
-        if (start < 0) { start = th; ori = o; }
-        ++cnt;
-        last = th;
-        if (cnt == kJobSegs || th + 1 - start >= kJobMaxSpan) { emit(start, th + 1); start = -1; cnt = 0; }
-      }
-    }
-    if (start >= 0) emit(start, last + 1);
-  }
-  if (njobs == 0) { ori = 0; emit(0, 0); }  // untouched tile: one exclusive job that stores zeros
-  if (!FILL) a.count[gid] = njobs;
-}
-
-__device__ __forceinline__ float2 lds_v(unsigned addr) {
-  float2 r;
-  asm volatile("ld.volatile.shared.v2.f32 {%0,%1}, [%2];" : "=f"(r.x), "=f"(r.y) : "r"(addr) : "memory");
-  return r;
-}
-__device__ __forceinline__ void sts_v(unsigned addr, float2 v) {
-  asm volatile("st.volatile.shared.v2.f32 [%0], {%1,%2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
-}
-
-template <int W>
-__device__ __forceinline__ void kernel_weights(const KerPoly& kp, float d, float (&wt)[W]) {
-  float d2 = d * d;
-#pragma unroll
-  for (int j = 0; j < W / 2; ++j) {
-    float e = kp.E[j][3], o = kp.O[j][3];
-#pragma unroll
-    for (int q = 2; q >= 0; --q) {
-      e = fmaf(e, d2, kp.E[j][q]);
-      o = fmaf(o, d2, kp.O[j][q]);
-    }
-    wt[j] = fmaf(d, o, e);
-    wt[W - 1 - j] = fmaf(-d, o, e);
-  }
-}
-
-template <int W>
-__device__ __forceinline__ void kernel_weights_r(const float (&E)[W / 2][kPolyHalf], const float (&O)[W / 2][kPolyHalf], float d,
-                                                 float (&wt)[W]) {
-  float d2 = d * d;
-#pragma unroll
-  for (int j = 0; j < W / 2; ++j) {
-    float e = E[j][3], o = O[j][3];
-#pragma unroll
-    for (int q = 2; q >= 0; --q) {
-      e = fmaf(e, d2, E[j][q]);
-      o = fmaf(o, d2, O[j][q]);
-    }
-    wt[j] = fmaf(d, o, e);
-    wt[W - 1 - j] = fmaf(-d, o, e);
-  }
-}
-
-struct SpreadArgs {
-  SpreadGeom g;
-  KerPoly kp;
-  const uint2* jobs;   // jobs of this launch
-  long long njobs;
-  const float2* S;     // [h/2+1][ntheta][WQ]
-  int WQ;
-  float2* G;           // [planes in batch][M][M]
-  int p0;              // first plane of the batch
-  const unsigned* multi;  // tiles of the batch's planes that several jobs write (k_zero_tiles)
-  long long nmulti;
-};
-
-// zero the tiles that receive atomic adds from several jobs: one warp per entry of the plan's list of such tiles
-// (entry = plane << 18 | ty << 9 | tx, built once from the job counts)
-__global__ void k_zero_tiles(SpreadArgs a) {
-  const int lane = threadIdx.x & 31;
-  long long j = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (j >= a.nmulti) return;
-  const unsigned e = a.multi[j];
-  const int M = a.g.M;
-  int tx = e & 0x1ff, ty = (e >> 9) & 0x1ff, p = e >> 18;
-  float2* Gp = a.G + (size_t)(p - a.p0) * M * M;
-  const int x0 = tx * kTile, y0 = ty * kTile;
-  for (int r = 0; r < kTile && y0 + r < M; ++r)
-    for (int c = lane; c < kTile && x0 + c < M; c += 32) Gp[(size_t)(y0 + r) * M + x0 + c] = make_float2(0.f, 0.f);
-}
-
-// Spreading of one job.  The warp owns a private storage tile [kTile][kTP] in shared memory; a sample is visited
-// iff its W x W footprint meets the kTile x kTile cells, and every tap is bounds-tested against the tile (the variant
-// with a kernel halo around the tile and no tests, kHalo, halves the resident warps and is slower).
-//
-// Lane roles: half-warp h holds two slots of W lanes; lane j of a slot owns tap column j of the slot's current
-// sample (along the MAJOR axis: x for x-dominant lines, y for y-dominant lines, whose jobs work on the transposed
-// tile) and walks the W taps of the minor axis.  The four slots take samples q apart on the same line,
-// q = ceil(W / sqrt 2): their footprints are disjoint (no lost update inside one instruction), and for W = 6 the
-// two runs of 6 contiguous cells of a half-warp sit 7..10 columns apart in rows whose pitch is a multiple of 16:
-// 12 distinct banks per 128-byte wavefront, no conflicts by construction.
-template <int W>
-__global__ void __launch_bounds__(32) k_spread(SpreadArgs a) {
-  extern __shared__ float2 tile[];
-  constexpr int H = kHalo ? W - 1 : 0;               // low-side halo of the storage (0: taps are bounds-tested)
-  constexpr int ROWS = kHalo ? kTile + 2 * W - 2 : kTile;
-  const SpreadGeom& g = a.g;
-  const int Q = g.kstride;  // sample distance between slots (footprints disjoint)
-  const int lane = threadIdx.x;
-  const long long jid = blockIdx.x;
-  const unsigned tile_addr = (unsigned)__cvta_generic_to_shared(tile);
-  const uint2 jb = a.jobs[jid];
-  const int tx = jb.x & 0x1ff, ty = (jb.x >> 9) & 0x1ff, th0 = jb.x >> 18;
-  const int nth = jb.y & 0x3ff, usex = (jb.y >> 10) & 7, usey = (jb.y >> 13) & 7;
-  const unsigned flags = (jb.y >> 16) & 3u;
-  const int p = (jb.y >> 18) & 0x1fff;
-  const bool ydom = (jb.y >> 31) != 0;
-  const int kv = p == g.hh ? -g.hh : p;
-  const double rho = g.rho_unit * kv;
-  const int mx0 = tx * kTile - g.M / 2, my0 = ty * kTile - g.M / 2;
-  const int hw = g.w / 2;
-
-  // lane role
-  const int hl = lane & 15, slot2 = hl / W, j1 = hl - slot2 * W;
-  const bool role = slot2 < 2;
-  const int sidx = 2 * (lane >> 4) + slot2;
-  const int slot_lane0 = role ? lane - j1 : lane;  // first lane of this lane's slot
-  float cE[kPolyHalf], cO[kPolyHalf];  // this lane's major-axis tap polynomial: E(d^2) + d O(d^2)
-  {
-    const int jj = role ? min(j1, W - 1 - j1) : 0;
-    const float sg = j1 < W / 2 ? 1.f : -1.f;
-#pragma unroll
-    for (int q = 0; q < kPolyHalf; ++q) {
-      cE[q] = a.kp.E[jj][q];
-      cO[q] = sg * a.kp.O[jj][q];
-    }
-  }
-
-  for (int i = lane; i < ROWS * kTP; i += 32) tile[i] = make_float2(0.f, 0.f);
-  float2* stg = tile + ROWS * kTP;  // [2][kStage] samples of the current / next line
-  int sb = 0;
-  __syncwarp();
-
-  const float2* Sp = a.S + (size_t)p * g.ntheta * a.WQ;
-  for (int tb = th0; tb < th0 + nth; tb += 32) {
-    const int th = tb + lane;
-    const bool tvalid = th < th0 + nth;
-    double2 cs = tvalid ? g.cs[th] : make_double2(1.0, 0.0);
-    const float c = (float)cs.x, s = (float)cs.y;
-    for (int sy = -1; sy <= 1; ++sy) {
-      if (!(usey >> (sy + 1) & 1)) continue;
-      const double oyd = -rho * cs.x - my0 + (double)sy * g.M;
-      for (int sx = -1; sx <= 1; ++sx) {
-        if (!(usex >> (sx + 1) & 1)) continue;
-        const double oxd = rho * cs.y - mx0 + (double)sx * g.M;
-        int ka = 1, kb = 0;
-        if (tvalid) clip_line<W>((float)oxd, (float)oyd, c, s, g.a1, hw, ka, kb);
-        // position of sample ka relative to the tile, in double (large terms cancel), then fp32
-        const double u0 = (double)g.a1 * ka;
-        const float p0x = (float)(oxd + u0 * cs.x), p0y = (float)(oyd + u0 * cs.y);
-        // major / minor axes of this job
-        const float lM0 = ydom ? p0y : p0x, lm0 = ydom ? p0x : p0y, lcM = ydom ? s : c, lcm = ydom ? c : s;
-        unsigned mask = __ballot_sync(0xffffffffu, ka <= kb);
-        if (!mask) continue;
-        // lines of this batch, one after the other; the samples of the NEXT line are fetched into registers while
-        // the current line is spread, then parked in the staging buffer (double-buffered)
-        int src = __ffs(mask) - 1;
-        int ska = __shfl_sync(0xffffffffu, ka, src), n = __shfl_sync(0xffffffffu, kb, src) - ska + 1;
-        const float2* Srow = Sp + (size_t)(tb + src) * a.WQ + hw + ska;
-        stg[sb * kStage + lane] = lane < n ? __ldg(&Srow[lane]) : make_float2(0.f, 0.f);
-        stg[sb * kStage + lane + 32] = lane + 32 < n ? __ldg(&Srow[lane + 32]) : make_float2(0.f, 0.f);
-        while (true) {
-          const float aM = g.a1 * __shfl_sync(0xffffffffu, lcM, src), am = g.a1 * __shfl_sync(0xffffffffu, lcm, src);
-          const float M0 = __shfl_sync(0xffffffffu, lM0, src), m0 = __shfl_sync(0xffffffffu, lm0, src);
-          mask &= mask - 1;
-          const bool more = mask != 0;
-          int nsrc = 0, nska = 0, nn = 0;
-          const float2* nSrow = Srow;
-          float2 nv0 = make_float2(0.f, 0.f), nv1 = nv0;
-          if (more) {
-            nsrc = __ffs(mask) - 1;
-            nska = __shfl_sync(0xffffffffu, ka, nsrc);
-            nn = __shfl_sync(0xffffffffu, kb, nsrc) - nska + 1;
-            nSrow = Sp + (size_t)(tb + nsrc) * a.WQ + hw + nska;
-            if (lane < nn) nv0 = __ldg(&nSrow[lane]);
-            if (lane + 32 < nn) nv1 = __ldg(&nSrow[lane + 32]);
-          }
-          __syncwarp();
-          for (int seg = 0; seg < n; seg += kStage) {
-            if (seg > 0) {  // long lines (small a1): later segments are fetched in place
-              __syncwarp();
-              stg[sb * kStage + lane] = seg + lane < n ? __ldg(&Srow[seg + lane]) : make_float2(0.f, 0.f);
-              stg[sb * kStage + lane + 32] = seg + lane + 32 < n ? __ldg(&Srow[seg + lane + 32]) : make_float2(0.f, 0.f);
-              __syncwarp();
-            }
-            const int nseg = min(n - seg, kStage);
-            // 4*kNU slots (kNU per lane) take samples Qe apart; one sweep of Qe steps covers the segment
-            const int Qe = max(Q, (nseg + 4 * kNU - 1) / (4 * kNU));
-#pragma unroll 1
-            for (int it = 0; it < Qe; ++it) {
-              float2 acc[kNU][W];
-              float wm[kNU][W];
-              float2 vw[kNU];
-              unsigned ad[kNU];
-              bool ok[kNU];
-              int rw0[kNU];
-#pragma unroll
-              for (int u = 0; u < kNU; ++u) {
-                const int kk = (sidx + 4 * u) * Qe + it;
-                const float fk = (float)(seg + kk);
-                const float tM = fmaf(fk, aM, M0), tm = fmaf(fk, am, m0);
-                const float cf = ceilf(tM - 0.5f * W), rf = ceilf(tm - 0.5f * W);
-                const int col0 = (int)cf, row0 = (int)rf;
-                ok[u] = role && kk < nseg && (unsigned)(col0 + W - 1) < (unsigned)(kTile + W - 1) &&
-                        (unsigned)(row0 + W - 1) < (unsigned)(kTile + W - 1);
-                if (!kHalo) ok[u] = ok[u] && (unsigned)(col0 + j1) < (unsigned)kTile;  // this lane's tap column
-                rw0[u] = row0;
-                const float2 v = stg[sb * kStage + (kk & (kStage - 1))];
-                // this lane's tap polynomial at both offsets: its own major-axis weight, and minor-axis weight j1
-                // of the slot's sample, which the W lanes of the slot then exchange
-                const float dM = tM - cf - (0.5f * W - 0.5f), dm = tm - rf - (0.5f * W - 0.5f);
-                const float dM2 = dM * dM, dm2 = dm * dm;
-                float eM = cE[3], oM = cO[3], em = cE[3], om = cO[3];
-#pragma unroll
-                for (int q = 2; q >= 0; --q) {
-                  eM = fmaf(eM, dM2, cE[q]);
-                  oM = fmaf(oM, dM2, cO[q]);
-                  em = fmaf(em, dm2, cE[q]);
-                  om = fmaf(om, dm2, cO[q]);
-                }
-                const float wM = fmaf(dM, oM, eM), wmine = fmaf(dm, om, em);
-#pragma unroll
-                for (int j2 = 0; j2 < W; ++j2) wm[u][j2] = __shfl_sync(0xffffffffu, wmine, slot_lane0 + j2);
-                vw[u] = make_float2(v.x * wM, v.y * wM);
-                ad[u] = tile_addr + (unsigned)((row0 + H) * kTP + col0 + H + j1) * 8u;
-              }
-#pragma unroll
-              for (int u = 0; u < kNU; ++u)
-#pragma unroll
-                for (int j2 = 0; j2 < W; ++j2)
-                  if (ok[u] && (kHalo || (unsigned)(rw0[u] + j2) < (unsigned)kTile)) acc[u][j2] = lds_v(ad[u] + j2 * (kTP * 8));
-#pragma unroll
-              for (int u = 0; u < kNU; ++u)
-#pragma unroll
-                for (int j2 = 0; j2 < W; ++j2) {
-                  acc[u][j2].x = fmaf(vw[u].x, wm[u][j2], acc[u][j2].x);
-                  acc[u][j2].y = fmaf(vw[u].y, wm[u][j2], acc[u][j2].y);
-                }
-#pragma unroll
-              for (int u = 0; u < kNU; ++u)
-#pragma unroll
-                for (int j2 = 0; j2 < W; ++j2)
-                  if (ok[u] && (kHalo || (unsigned)(rw0[u] + j2) < (unsigned)kTile)) sts_v(ad[u] + j2 * (kTP * 8), acc[u][j2]);
-            }
-          }
-          if (!more) break;
-          sb ^= 1;
-          stg[sb * kStage + lane] = nv0;
-          stg[sb * kStage + lane + 32] = nv1;
-          src = nsrc;
-          ska = nska;
-          n = nn;
-          Srow = nSrow;
-        }
-        __syncwarp();
-      }
-    }
-  }
-  __syncwarp();
-  // y-dominant jobs worked on the transposed tile: transpose the owned square in place (diagonal sweeps: lane i swaps
-  // (i, i+r) with (i+r, i); both accesses of an instruction touch distinct banks)
-  if (ydom) {
-    for (int r = 1; r <= kTile / 2; ++r) {
-      for (int i = lane; i < kTile; i += 32) {
-        if (2 * r == kTile && i >= kTile / 2) continue;
-        int j = i + r;
-        if (j >= kTile) j -= kTile;
-        const unsigned a1 = tile_addr + (unsigned)((i + H) * kTP + j + H) * 8u;
-        const unsigned a2 = tile_addr + (unsigned)((j + H) * kTP + i + H) * 8u;
-        float2 u = lds_v(a1), v = lds_v(a2);
-        sts_v(a1, v);
-        sts_v(a2, u);
-      }
-    }
-    __syncwarp();
-  }
-  const int M = g.M, x0 = tx * kTile, y0 = ty * kTile;
-  float2* Gp = a.G + (size_t)(p - a.p0) * M * M;
-  if (flags & kJobExclusive) {
-    for (int r = 0; r < kTile && y0 + r < M; ++r)
-      for (int cc = lane; cc < kTile && x0 + cc < M; cc += 32)
-        Gp[(size_t)(y0 + r) * M + x0 + cc] = lds_v(tile_addr + (unsigned)((r + H) * kTP + cc + H) * 8u);
-  } else {
-    for (int r = 0; r < kTile && y0 + r < M; ++r)
-      for (int cc = lane; cc < kTile && x0 + cc < M; cc += 32) {
-        float2 v = lds_v(tile_addr + (unsigned)((r + H) * kTP + cc + H) * 8u);
-        if (v.x != 0.f || v.y != 0.f) atomicAdd(&Gp[(size_t)(y0 + r) * M + x0 + cc], v);
-      }
-  }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
