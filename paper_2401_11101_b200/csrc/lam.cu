@@ -639,7 +639,7 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
     }
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;
-      const size_t sm = (size_t)kTS * kTS * sizeof(float2) + (size_t)kSW * 32 * sizeof(LineParams);
+      const size_t sm = spread_smem();
       cudaFuncSetAttribute(k_spread<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
       k_spread<W><<<(unsigned)sa.njobs, 32 * kSW, sm, s>>>(sa);
       note_launch();

@@ -23,6 +23,7 @@
 // first (k_zero_tiles) and merged with red.global.add.
 #pragma once
 #include <cstdint>
+#include <type_traits>
 #include <cuda_runtime.h>
 
 #include "lam_math.h"
@@ -35,7 +36,6 @@ constexpr int kJobRanges = 6;      // theta ranges per job
 constexpr int kJobMaxLines = 256;  // lines per job; a tile crossed by more lines is split over several jobs
 constexpr int kRangeGap = 32;      // non-crossing thetas tolerated inside a range
 constexpr int kRangeMaxLen = 2047; // 11 bits
-constexpr int kNI = 6;             // samples of one line per lane and sweep (W / (a1 / sqrt 2) + 1 for a1 = 2, W = 6)
 constexpr int kMaxW = 8;
 
 struct SpreadGeom {
@@ -233,6 +233,38 @@ __global__ void k_zero_tiles(SpreadArgs a) {
   }
 }
 
+__device__ __forceinline__ void cp_async8(unsigned dst, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+template <int OFF>
+__device__ __forceinline__ float2 lds_f2(unsigned addr) {
+  float2 r;
+  asm volatile("ld.shared.v2.f32 {%0,%1}, [%2+%3];" : "=f"(r.x), "=f"(r.y) : "r"(addr), "n"(OFF) : "memory");
+  return r;
+}
+template <int OFF>
+__device__ __forceinline__ void sts_f2(unsigned addr, float2 v) {
+  asm volatile("st.shared.v2.f32 [%0+%3], {%1,%2};" ::"r"(addr), "f"(v.x), "f"(v.y), "n"(OFF) : "memory");
+}
+
+__host__ __device__ constexpr int j_off(int j);
+template <int J, int N, class F>
+__device__ __forceinline__ void static_for(F&& f) {
+  if constexpr (J < N) {
+    f(std::integral_constant<int, J>{});
+    static_for<J + 1, N>(f);
+  }
+}
+constexpr int kStg = 64;   // samples of one line staged per sweep
+
+// dynamic shared memory of k_spread: tile + per-warp line parameters + per-warp sample staging
+constexpr size_t spread_smem() { return (size_t)kTS * kTS * 8 + (size_t)kSW * 32 * 32 + (size_t)kSW * 2 * kStg * 8 + 2 * (kMaxW / 2) * kPolyHalf * 4; }
+
+__host__ __device__ constexpr int j_off(int j) { return j * kTS * 8; }  // byte offset of tap row j in a tile column
+
 struct LineParams {   // one line (theta, periodic image) clipped against a strip; 32 bytes
   float PM0, Pm0;     // position of sample ka relative to the strip's first cell (major, minor)
   float aM, am;       // step per sample
@@ -248,6 +280,9 @@ __global__ void __launch_bounds__(32 * kSW) k_spread(SpreadArgs a) {
   float2* tile = smem;                                            // [kTS][kTS]: [minor][major]
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   LineParams* lp = reinterpret_cast<LineParams*>(smem + kTS * kTS) + wid * 32;
+  float2* stg_all = smem + kTS * kTS + kSW * 32 * (sizeof(LineParams) / sizeof(float2));
+  float2* stg = stg_all + wid * 2 * kStg;  // [2][kStg] samples
+  const unsigned stg_addr = (unsigned)__cvta_generic_to_shared(stg);
   const SpreadGeom& g = a.g;
   const Job jb = a.jobs[blockIdx.x];
   const int tx = jb.w[0] & 0xff, ty = (jb.w[0] >> 8) & 0xff, p = (jb.w[0] >> 16) & 0x1fff;
@@ -267,7 +302,25 @@ __global__ void __launch_bounds__(32 * kSW) k_spread(SpreadArgs a) {
   __syncthreads();
 
   const float2* Sp = a.S + (size_t)p * g.ntheta * a.WQ;
-  float2* mycol = tile + col;
+  const unsigned mycol_addr = (unsigned)__cvta_generic_to_shared(tile + col);
+  // polynomial coefficients of the kernel pieces, pinned in registers (the compiler would re-read the constant bank
+  // in every iteration otherwise)
+  float cE[W / 2][kPolyHalf], cO[W / 2][kPolyHalf];
+  {
+    float* kps = reinterpret_cast<float*>(stg_all + kSW * 2 * kStg);
+    if (threadIdx.x < (kMaxW / 2) * kPolyHalf) {
+      kps[threadIdx.x] = (&a.kp.E[0][0])[threadIdx.x];
+      kps[(kMaxW / 2) * kPolyHalf + threadIdx.x] = (&a.kp.O[0][0])[threadIdx.x];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < W / 2; ++j)
+#pragma unroll
+      for (int q = 0; q < kPolyHalf; ++q) {
+        cE[j][q] = reinterpret_cast<volatile float*>(kps)[j * kPolyHalf + q];
+        cO[j][q] = reinterpret_cast<volatile float*>(kps)[(kMaxW / 2) * kPolyHalf + j * kPolyHalf + q];
+      }
+  }
 
   for (int phase = 0; phase < 2; ++phase) {
     if (phase == 0 ? !hasx : !hasy) continue;
@@ -285,8 +338,9 @@ __global__ void __launch_bounds__(32 * kSW) k_spread(SpreadArgs a) {
       }
       __syncthreads();
     }
+#pragma unroll 1
     for (int ri = 0; ri < nranges; ++ri) {
-      const unsigned rw = jb.w[2 + ri];
+      const unsigned rw = __ldg(&a.jobs[blockIdx.x].w[2 + ri]);
       if (((rw >> 25) & 1u) != (unsigned)phase) continue;
       const int rs = rw & 0x3fff, rend = rs + (int)((rw >> 14) & 0x7ff);
       for (int tb = rs; tb < rend; tb += 32) {
@@ -295,9 +349,11 @@ __global__ void __launch_bounds__(32 * kSW) k_spread(SpreadArgs a) {
         const double2 cs = tvalid ? g.cs[th] : make_double2(1.0, 0.0);
         const double cMd = ydom ? cs.y : cs.x, cmd = ydom ? cs.x : cs.y;
         const float cM = (float)cMd, cm = (float)cmd;
+#pragma unroll 1
         for (int sy = -1; sy <= 1; ++sy) {
           if (!(usey >> (sy + 1) & 1)) continue;
           const double oyd = -rho * cs.x - my0 + (double)sy * g.M;
+#pragma unroll 1
           for (int sx = -1; sx <= 1; ++sx) {
             if (!(usex >> (sx + 1) & 1)) continue;
             const double oxd = rho * cs.y - mx0 + (double)sx * g.M;
@@ -322,99 +378,129 @@ __global__ void __launch_bounds__(32 * kSW) k_spread(SpreadArgs a) {
                 make_float4(me.inv, __int_as_float(me.n), __int_as_float(me.soff), 0.f);
             unsigned mask = __ballot_sync(0xffffffffu, hit);
             __syncwarp();
-            // lines of this batch one after the other; the samples of the NEXT line are fetched into registers while the
-            // current line is spread
-            float cPM0 = 0.f, cPm0 = 0.f, caM = 0.f, cam = 0.f;
-            int cis = 0, ccnt = 0, cNI = 0, csoff = 0;
-            float2 cv[kNI];
-            bool have = false;
-            while (true) {
-              const bool more = mask != 0;
-              float nPM0 = 0.f, nPm0 = 0.f, naM = 0.f, nam = 0.f;
-              int nis = 0, ncnt = 0, nNI = 0, nsoff = 0;
-              float2 nv[kNI];
-              if (more) {
-                const int src = __ffs(mask) - 1;
+            // lines of this batch one after the other; the samples of the NEXT line are copied into the other staging
+            // buffer (cp.async) while the current line is spread
+            int buf = 0;
+            auto stage = [&](int src, int bsel) {   // first kStg samples of line `src` -> stg[bsel]
+              const int n = lp[src].n;
+              const float2* row = Sp + lp[src].soff;
+              const unsigned dst = stg_addr + (unsigned)(bsel * kStg + 2 * lane) * 8u;
+              if (2 * lane < n) cp_async8(dst, row + 2 * lane);
+              if (2 * lane + 1 < n) cp_async8(dst + 8u, row + 2 * lane + 1);
+              cp_async_commit();
+            };
+            int cur = -1;
+            if (mask) {
+              cur = __ffs(mask) - 1;
+              mask &= mask - 1;
+              stage(cur, buf);
+            }
+            while (cur >= 0) {
+              cp_async_wait_all();
+              __syncwarp();
+              int nxt = -1;
+              if (mask) {
+                nxt = __ffs(mask) - 1;
                 mask &= mask - 1;
-                const float4 q0 = reinterpret_cast<const float4*>(lp + src)[0];
-                const float4 q1 = reinterpret_cast<const float4*>(lp + src)[1];
-                nPM0 = q0.x; nPm0 = q0.y; naM = q0.z; nam = q0.w;
-                const int n = __float_as_int(q1.y);
-                nsoff = __float_as_int(q1.z);
-                const float uA = (fL - 0.5f * W - nPM0) * q1.x, uB = (fL + 0.5f * W - nPM0) * q1.x;
-                nis = max(0, (int)ceilf(fminf(uA, uB) - 1e-3f));
-                const int ie = min(n - 1, (int)floorf(fmaxf(uA, uB) + 1e-3f));
-                ncnt = ie - nis + 1;
-                nNI = __reduce_max_sync(0xffffffffu, ncnt);
-                const float2* src_row = Sp + nsoff + nis;
-#pragma unroll
-                for (int i = 0; i < kNI; ++i) nv[i] = i < ncnt ? __ldg(src_row + i) : make_float2(0.f, 0.f);
+                stage(nxt, buf ^ 1);
               }
-              if (have) {
-                for (int i0 = 0; i0 < cNI; i0 += kNI) {
-                  if (i0 > 0) {  // long runs (a1 < 2): later sweeps are fetched in place
+              const float4 q0 = reinterpret_cast<const float4*>(lp + cur)[0];
+              const float4 q1 = reinterpret_cast<const float4*>(lp + cur)[1];
+              const float PM0 = q0.x, Pm0 = q0.y, aM = q0.z, am = q0.w;
+              const int n = __float_as_int(q1.y);
+              const float uA = (fL - 0.5f * W - PM0) * q1.x, uB = (fL + 0.5f * W - PM0) * q1.x;
+              const int is = max(0, (int)ceilf(fminf(uA, uB) - 1e-3f));
+              const int ie = min(n - 1, (int)floorf(fmaxf(uA, uB) + 1e-3f));
+              for (int seg = 0; seg < n; seg += kStg) {
+                if (seg > 0) {  // long runs (a1 < 2): later segments are fetched in place
+                  __syncwarp();
+                  const float2* row = Sp + __float_as_int(q1.z) + seg;
+                  stg[buf * kStg + 2 * lane] = seg + 2 * lane < n ? __ldg(row + 2 * lane) : make_float2(0.f, 0.f);
+                  stg[buf * kStg + 2 * lane + 1] = seg + 2 * lane + 1 < n ? __ldg(row + 2 * lane + 1) : make_float2(0.f, 0.f);
+                  __syncwarp();
+                }
+                const int ls = max(is, seg), cnt = min(ie, seg + kStg - 1) - ls + 1;
+                const int NI = __reduce_max_sync(0xffffffffu, cnt);
+                const float2* sv = stg + buf * kStg + (ls - seg);
+                // software pipeline: the taps of pair i are loaded, the weights of pair i+1 are evaluated while those
+                // loads are in flight, then pair i is accumulated and stored
+                auto prep = [&](int i, float2& vw, float (&wm)[W], unsigned& addr, unsigned& rm) {
+                  const float fk = (float)(ls + i);
+                  const float2 P = __ffma2_rn(make_float2(fk, fk), make_float2(aM, am), make_float2(PM0, Pm0));
+                  const float xM = P.x - 0.5f * W, xm = P.y - 0.5f * W;
+                  const float cf = ceilf(xM), rf = ceilf(xm);
+                  const int j1 = lane - (int)cf;
+                  const int r0 = (int)rf;
+                  const bool ok = i < cnt && (unsigned)j1 < (unsigned)W;
+                  const float2 v = sv[i < cnt ? i : 0];
+                  const float dM = (xM - cf) + 0.5f, dm = (xm - rf) + 0.5f;
+                  // E_j(d^2), O_j(d^2) of every half-tap j for both axes at once: .x major, .y minor
+                  const float2 d2 = __fmul2_rn(make_float2(dM, dm), make_float2(dM, dm));
+                  float2 e[W / 2], o[W / 2];
 #pragma unroll
-                    for (int i = 0; i < kNI; ++i) cv[i] = i0 + i < ccnt ? __ldg(Sp + csoff + cis + i0 + i) : make_float2(0.f, 0.f);
-                  }
+                  for (int j = 0; j < W / 2; ++j) {
+                    e[j] = make_float2(cE[j][3], cE[j][3]);
+                    o[j] = make_float2(cO[j][3], cO[j][3]);
 #pragma unroll
-                  for (int i = 0; i < kNI; ++i) {
-                    if (i0 + i >= cNI) break;
-                    const float fk = (float)(cis + i0 + i);
-                    const float PM = fmaf(fk, caM, cPM0), Pm = fmaf(fk, cam, cPm0);
-                    const float cf = ceilf(PM - 0.5f * W), rf = ceilf(Pm - 0.5f * W);
-                    const int j1 = lane - (int)cf, r0 = (int)rf;
-                    const bool ok = i0 + i < ccnt && (unsigned)j1 < (unsigned)W;
-                    const float dM = PM - cf - (0.5f * W - 0.5f), dm = Pm - rf - (0.5f * W - 0.5f);
-                    // E_j(d^2), O_j(d^2) of every half-tap j for both axes at once: .x major, .y minor
-                    const float2 d2 = __fmul2_rn(make_float2(dM, dm), make_float2(dM, dm));
-                    float2 e[W / 2], o[W / 2];
-#pragma unroll
-                    for (int j = 0; j < W / 2; ++j) {
-                      e[j] = make_float2(a.kp.E[j][3], a.kp.E[j][3]);
-                      o[j] = make_float2(a.kp.O[j][3], a.kp.O[j][3]);
-#pragma unroll
-                      for (int q = 2; q >= 0; --q) {
-                        e[j] = __ffma2_rn(e[j], d2, make_float2(a.kp.E[j][q], a.kp.E[j][q]));
-                        o[j] = __ffma2_rn(o[j], d2, make_float2(a.kp.O[j][q], a.kp.O[j][q]));
-                      }
-                    }
-                    // major axis: this lane's tap j1 of the sample; taps j and W-1-j share E, O with opposite sign of d
-                    const int jj = j1 < W / 2 ? j1 : W - 1 - j1;
-                    float eM = e[0].x, oM = o[0].x;
-#pragma unroll
-                    for (int j = 1; j < W / 2; ++j) {
-                      eM = jj == j ? e[j].x : eM;
-                      oM = jj == j ? o[j].x : oM;
-                    }
-                    const float wM = fmaf(j1 < W / 2 ? dM : -dM, oM, eM);
-                    const float2 vw = make_float2(cv[i].x * wM, cv[i].y * wM);
-                    float2* cell = mycol + r0 * kTS;
-#pragma unroll
-                    for (int j = 0; j < W / 2; ++j) {
-                      const float wlo = fmaf(dm, o[j].y, e[j].y), whi = fmaf(-dm, o[j].y, e[j].y);
-                      if (ok && (unsigned)(r0 + j) < (unsigned)kTS) {
-                        float2 c = cell[j * kTS];
-                        c.x = fmaf(vw.x, wlo, c.x);
-                        c.y = fmaf(vw.y, wlo, c.y);
-                        cell[j * kTS] = c;
-                      }
-                      if (ok && (unsigned)(r0 + W - 1 - j) < (unsigned)kTS) {
-                        float2 c = cell[(W - 1 - j) * kTS];
-                        c.x = fmaf(vw.x, whi, c.x);
-                        c.y = fmaf(vw.y, whi, c.y);
-                        cell[(W - 1 - j) * kTS] = c;
-                      }
+                    for (int q = 2; q >= 0; --q) {
+                      e[j] = __ffma2_rn(e[j], d2, make_float2(cE[j][q], cE[j][q]));
+                      o[j] = __ffma2_rn(o[j], d2, make_float2(cO[j][q], cO[j][q]));
                     }
                   }
+                  // major axis: this lane's tap j1 of the sample; taps j and W-1-j share E, O with opposite sign of d
+                  const int jj = j1 < W / 2 ? j1 : W - 1 - j1;
+                  float eM = e[0].x, oM = o[0].x;
+#pragma unroll
+                  for (int j = 1; j < W / 2; ++j) {
+                    eM = jj == j ? e[j].x : eM;
+                    oM = jj == j ? o[j].x : oM;
+                  }
+                  const float wM = fmaf(j1 < W / 2 ? dM : -dM, oM, eM);
+                  vw = make_float2(v.x * wM, v.y * wM);
+#pragma unroll
+                  for (int j = 0; j < W / 2; ++j) {
+                    wm[j] = fmaf(dm, o[j].y, e[j].y);
+                    wm[W - 1 - j] = fmaf(-dm, o[j].y, e[j].y);
+                  }
+                  addr = mycol_addr + (unsigned)(r0 * (kTS * 8));
+                  // bit j: row r0 + j is inside the tile (and the pair exists)
+                  const int lo = min(max(-r0, 0), W), hi = min(max(kTS - r0, 0), W);
+                  rm = ok ? ((1u << hi) - 1u) & ~((1u << lo) - 1u) : 0u;
+                };
+                float2 vw, nvw, c[W];
+                float wm[W], nwm[W];
+                unsigned addr, naddr, rm, nrm;
+                prep(0, vw, wm, addr, rm);
+                static_for<0, W>([&](auto J) {
+                  if (rm >> J.value & 1u) c[J.value] = lds_f2<j_off(J.value)>(addr);
+                });
+                for (int i = 0;;) {
+                  const bool last = i + 1 >= NI;
+                  if (!last) prep(i + 1, nvw, nwm, naddr, nrm);
+#pragma unroll
+                  for (int j = 0; j < W; ++j) {
+                    c[j].x = fmaf(vw.x, wm[j], c[j].x);
+                    c[j].y = fmaf(vw.y, wm[j], c[j].y);
+                  }
+                  static_for<0, W>([&](auto J) {
+                    if (rm >> J.value & 1u) sts_f2<j_off(J.value)>(addr, c[J.value]);
+                  });
+                  if (last) break;
+                  ++i;
+                  vw = nvw;
+#pragma unroll
+                  for (int j = 0; j < W; ++j) wm[j] = nwm[j];
+                  addr = naddr;
+                  rm = nrm;
+                  static_for<0, W>([&](auto J) {
+                    if (rm >> J.value & 1u) c[J.value] = lds_f2<j_off(J.value)>(addr);
+                  });
                 }
               }
-              if (!more) break;
-              cPM0 = nPM0; cPm0 = nPm0; caM = naM; cam = nam;
-              cis = nis; ccnt = ncnt; cNI = nNI; csoff = nsoff;
-#pragma unroll
-              for (int i = 0; i < kNI; ++i) cv[i] = nv[i];
-              have = true;
+              cur = nxt;
+              buf ^= 1;
             }
+            __syncwarp();
           }
         }
       }
