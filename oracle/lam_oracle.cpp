@@ -14,11 +14,13 @@
 //           orc_forward_nudft  Eq. 5, exact NUDFT forward, tiny sizes (adjoint test).
 //   path B  orc_fbp_direct / orc_fp_direct   direct discretisation of Eq. 4 / Eq. 1 with linear
 //                              interpolation ("Linerec") — sanity + O(N^4) baseline.
+//           orc_fp_ray         Eq. 1-2 sampled along the beam, trilinear (ray-driven forward).
 //   path C  orc_fbp_gridded    USFFT of PAPER.md:130-142 (gridding, inverse 3D FFT, division by psi).
 //   path C' orc_fbp_gridded_slice   Eq. 9: exact x3 transform + 2D USFFT, one slice.
 //           orc_prep           dark/flat/-log, model of PAPER.md:99.
-// Pins: tests/test_oracle_*.py.  Path B has no independent pin beyond agreement with A ("parity
-// unpinned" for B; it is never used as a parity gate).
+// Pins: tests/test_oracle_*.py.  Path B: orc_fp_ray is pinned to analytic blob line integrals (P9b); the
+// voxel-driven pair is pinned as a transpose pair, by mass conservation and against A at the interpolation-error
+// level (a few per cent by construction: linear against trigonometric interpolation).  B is never a parity gate.
 //
 // Conventions: voxel x_a = i_a - n_a/2, detector u = j_u - c_u, v = j_v - c_v,
 // k_u in [-w/2,w/2), k_v in [-h/2,h/2), xi = (k_u/w) e_u + (k_v/h) e_v (cycles/voxel),
@@ -427,6 +429,45 @@ extern "C" void orc_fp_direct(const orc_geom* gp, const double* vol, double* pro
               q[(size_t)b * w + a] += (du ? au : 1 - au) * (dv ? av : 1 - av) * f;
             }
         }
+  }
+}
+
+// Ray-driven forward projection: the line integral of Eq. 1-2 sampled along the beam.
+// The two deltas of Eq. 2 fix (x.e_u, x.e_v) = (u, v); the line is x(t) = u e_u + v e_v + t e_b with the unit
+// beam direction e_b = e_u x e_v = (sin(theta) cos(phi), -cos(theta) cos(phi), -sin(phi)).  The integral is the sum over
+// unit steps t of mu(x(t)), mu trilinearly interpolated between voxel centres and zero outside the volume.
+extern "C" void orc_fp_ray(const orc_geom* gp, const double* vol, double* proj) {
+  const orc_geom& g = *gp;
+  int h = g.h, w = g.w, n = g.n, nz = g.nz;
+  const int T = (int)ceil(sqrt(0.5 * (double)n * n + 0.25 * (double)nz * nz)) + 2;
+  auto mu = [&](int i1, int i2, int i3) -> double {
+    if (i1 < 0 || i1 >= n || i2 < 0 || i2 >= n || i3 < 0 || i3 >= nz) return 0.0;
+    return vol[((size_t)i3 * n + i2) * n + i1];
+  };
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int th = 0; th < g.ntheta; ++th) {
+    double ct = cos(g.theta[th]), st = sin(g.theta[th]), cp = cos(g.phi), sp = sin(g.phi);
+    const double eu[3] = {ct, st, 0.0}, ev[3] = {st * sp, -ct * sp, cp}, eb[3] = {st * cp, -ct * cp, -sp};
+    for (int jv = 0; jv < h; ++jv)
+      for (int ju = 0; ju < w; ++ju) {
+        const double u = ju - g.cu, v = jv - g.cv;
+        double s = 0;
+        for (int t = -T; t <= T; ++t) {
+          // voxel index coordinates of the point (x1 = i1 - n/2, ...)
+          const double p1 = u * eu[0] + v * ev[0] + t * eb[0] + n / 2;
+          const double p2 = u * eu[1] + v * ev[1] + t * eb[1] + n / 2;
+          const double p3 = u * eu[2] + v * ev[2] + t * eb[2] + nz / 2;
+          const double f1 = floor(p1), f2 = floor(p2), f3 = floor(p3);
+          const int i1 = (int)f1, i2 = (int)f2, i3 = (int)f3;
+          if (i1 < -1 || i1 >= n || i2 < -1 || i2 >= n || i3 < -1 || i3 >= nz) continue;
+          const double a1 = p1 - f1, a2 = p2 - f2, a3 = p3 - f3;
+          for (int d3 = 0; d3 < 2; ++d3)
+            for (int d2 = 0; d2 < 2; ++d2)
+              for (int d1 = 0; d1 < 2; ++d1)
+                s += (d1 ? a1 : 1 - a1) * (d2 ? a2 : 1 - a2) * (d3 ? a3 : 1 - a3) * mu(i1 + d1, i2 + d2, i3 + d3);
+        }
+        proj[((size_t)th * h + jv) * w + ju] = s;
+      }
   }
 }
 

@@ -18,7 +18,7 @@ _LIB = os.path.join(_HERE, "liblam_oracle.so")
 def build(force=False):
     """Compile the oracle with g++ (no fast-math).  Building the checker is not using it."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared",
+        subprocess.check_call(["g++", "-O3", "-std=c++17", "-fopenmp", "-fPIC", "-shared",
                                "-o", _LIB, _SRC])
     return _LIB
 
@@ -174,6 +174,16 @@ def fp_direct(geom, vol):
     out = np.empty((geom.ntheta, geom.h, geom.w))
     g = geom._c(None)
     lib().orc_fp_direct(C.byref(g), _p(vol), _p(out))
+    return out
+
+
+def fp_ray(geom, vol):
+    """Ray-driven forward projection (Eq. 1-2): unit steps along the beam, trilinear."""
+    vol = np.ascontiguousarray(vol, dtype=np.float64)
+    assert vol.shape == (geom.nz, geom.n, geom.n)
+    out = np.empty((geom.ntheta, geom.h, geom.w))
+    g = geom._c(None)
+    lib().orc_fp_ray(C.byref(g), _p(vol), _p(out))
     return out
 
 

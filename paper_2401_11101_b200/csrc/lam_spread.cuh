@@ -30,7 +30,14 @@
 
 namespace lam {
 
-constexpr int kSW = 2;             // warps per job = strips of 32 major-axis cells
+#ifndef LAM_SW
+#define LAM_SW 1
+#endif
+#ifndef LAM_PIPE
+#define LAM_PIPE 0
+#endif
+constexpr int kSW = LAM_SW;        // warps per job = strips of 32 major-axis cells
+constexpr bool kPipe = LAM_PIPE;   // software-pipelined pair loop (more registers) or the plain one (more warps)
 constexpr int kTS = 32 * kSW;      // tile edge (fine-grid cells)
 constexpr int kJobRanges = 6;      // theta ranges per job
 constexpr int kJobMaxLines = 256;  // lines per job; a tile crossed by more lines is split over several jobs
@@ -233,12 +240,6 @@ __global__ void k_zero_tiles(SpreadArgs a) {
   }
 }
 
-__device__ __forceinline__ void cp_async8(unsigned dst, const void* src) {
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
-
 template <int OFF>
 __device__ __forceinline__ float2 lds_f2(unsigned addr) {
   float2 r;
@@ -250,7 +251,6 @@ __device__ __forceinline__ void sts_f2(unsigned addr, float2 v) {
   asm volatile("st.shared.v2.f32 [%0+%3], {%1,%2};" ::"r"(addr), "f"(v.x), "f"(v.y), "n"(OFF) : "memory");
 }
 
-__host__ __device__ constexpr int j_off(int j);
 template <int J, int N, class F>
 __device__ __forceinline__ void static_for(F&& f) {
   if constexpr (J < N) {
@@ -258,10 +258,6 @@ __device__ __forceinline__ void static_for(F&& f) {
     static_for<J + 1, N>(f);
   }
 }
-constexpr int kStg = 64;   // samples of one line staged per sweep
-
-// dynamic shared memory of k_spread: tile + per-warp line parameters + per-warp sample staging
-constexpr size_t spread_smem() { return (size_t)kTS * kTS * 8 + (size_t)kSW * 32 * 32 + (size_t)kSW * 2 * kStg * 8 + 2 * (kMaxW / 2) * kPolyHalf * 4; }
 
 __host__ __device__ constexpr int j_off(int j) { return j * kTS * 8; }  // byte offset of tap row j in a tile column
 
@@ -274,15 +270,26 @@ struct LineParams {   // one line (theta, periodic image) clipped against a stri
   int pad;
 };
 
+// per-warp record of the <= 32 samples of the current line segment (what depends on the sample only, evaluated once
+// per sample by lane = sample and read by the lanes = columns): value, minor-axis weights, first minor row + row mask
+struct LineRec {
+  float2 v[32];
+  float wm[kMaxW][32];
+  unsigned pk[32];   // (r0 & 0xff) | rowmask << 8
+};
+
+// dynamic shared memory of k_spread: tile + per-warp line parameters + per-warp sample records + kernel coefficients
+constexpr size_t spread_smem() {
+  return (size_t)kTS * kTS * 8 + (size_t)kSW * 32 * sizeof(LineParams) + (size_t)kSW * sizeof(LineRec) + 2 * (kMaxW / 2) * kPolyHalf * 4;
+}
+
 template <int W>
-__global__ void __launch_bounds__(32 * kSW) k_spread(SpreadArgs a) {
+__global__ void __launch_bounds__(32 * kSW, kSW == 1 ? 20 : 6) k_spread(SpreadArgs a) {
   extern __shared__ float2 smem[];
   float2* tile = smem;                                            // [kTS][kTS]: [minor][major]
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   LineParams* lp = reinterpret_cast<LineParams*>(smem + kTS * kTS) + wid * 32;
-  float2* stg_all = smem + kTS * kTS + kSW * 32 * (sizeof(LineParams) / sizeof(float2));
-  float2* stg = stg_all + wid * 2 * kStg;  // [2][kStg] samples
-  const unsigned stg_addr = (unsigned)__cvta_generic_to_shared(stg);
+  LineRec* rec = reinterpret_cast<LineRec*>(reinterpret_cast<LineParams*>(smem + kTS * kTS) + kSW * 32) + wid;
   const SpreadGeom& g = a.g;
   const Job jb = a.jobs[blockIdx.x];
   const int tx = jb.w[0] & 0xff, ty = (jb.w[0] >> 8) & 0xff, p = (jb.w[0] >> 16) & 0x1fff;
@@ -299,15 +306,11 @@ __global__ void __launch_bounds__(32 * kSW) k_spread(SpreadArgs a) {
     float4* t4 = reinterpret_cast<float4*>(tile);
     for (int i = threadIdx.x; i < kTS * kTS / 2; i += 32 * kSW) t4[i] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
-  __syncthreads();
-
-  const float2* Sp = a.S + (size_t)p * g.ntheta * a.WQ;
-  const unsigned mycol_addr = (unsigned)__cvta_generic_to_shared(tile + col);
-  // polynomial coefficients of the kernel pieces, pinned in registers (the compiler would re-read the constant bank
-  // in every iteration otherwise)
-  float cE[W / 2][kPolyHalf], cO[W / 2][kPolyHalf];
+  // polynomial coefficients (E_j[q], O_j[q]) of the kernel pieces, pinned in registers: read back from shared memory so
+  // that the compiler cannot re-read the constant bank in every iteration
+  float2 cEO[W / 2][kPolyHalf];
   {
-    float* kps = reinterpret_cast<float*>(stg_all + kSW * 2 * kStg);
+    float* kps = reinterpret_cast<float*>(reinterpret_cast<LineRec*>(reinterpret_cast<LineParams*>(smem + kTS * kTS) + kSW * 32) + kSW);
     if (threadIdx.x < (kMaxW / 2) * kPolyHalf) {
       kps[threadIdx.x] = (&a.kp.E[0][0])[threadIdx.x];
       kps[(kMaxW / 2) * kPolyHalf + threadIdx.x] = (&a.kp.O[0][0])[threadIdx.x];
@@ -316,11 +319,23 @@ __global__ void __launch_bounds__(32 * kSW) k_spread(SpreadArgs a) {
 #pragma unroll
     for (int j = 0; j < W / 2; ++j)
 #pragma unroll
-      for (int q = 0; q < kPolyHalf; ++q) {
-        cE[j][q] = reinterpret_cast<volatile float*>(kps)[j * kPolyHalf + q];
-        cO[j][q] = reinterpret_cast<volatile float*>(kps)[(kMaxW / 2) * kPolyHalf + j * kPolyHalf + q];
-      }
+      for (int q = 0; q < kPolyHalf; ++q)
+        cEO[j][q] = make_float2(reinterpret_cast<volatile float*>(kps)[j * kPolyHalf + q],
+                                reinterpret_cast<volatile float*>(kps)[(kMaxW / 2) * kPolyHalf + j * kPolyHalf + q]);
   }
+  // (E_j(d^2), O_j(d^2)) of every half-tap j, packed: tap j has weight E_j + d O_j, tap W-1-j has E_j - d O_j
+  auto pieces = [&](float d, float2 (&eo)[W / 2]) {
+    const float d2 = d * d;
+#pragma unroll
+    for (int j = 0; j < W / 2; ++j) {
+      eo[j] = cEO[j][kPolyHalf - 1];
+#pragma unroll
+      for (int q = kPolyHalf - 2; q >= 0; --q) eo[j] = __ffma2_rn(eo[j], make_float2(d2, d2), cEO[j][q]);
+    }
+  };
+
+  const float2* Sp = a.S + (size_t)p * g.ntheta * a.WQ;
+  const unsigned mycol_addr = (unsigned)__cvta_generic_to_shared(tile + col);
 
   for (int phase = 0; phase < 2; ++phase) {
     if (phase == 0 ? !hasx : !hasy) continue;
@@ -363,142 +378,146 @@ __global__ void __launch_bounds__(32 * kSW) k_spread(SpreadArgs a) {
             const bool hit = ka <= kb;
             // position of sample ka relative to the strip, in double (large terms cancel), then fp32
             const double u0 = (double)g.a1 * ka;
-            LineParams me;
-            me.PM0 = (float)(oMd + u0 * cMd);
-            me.Pm0 = (float)(omd + u0 * cmd);
-            me.aM = g.a1 * cM;
-            me.am = g.a1 * cm;
-            me.inv = 1.0f / me.aM;
-            me.n = kb - ka + 1;
-            me.soff = th * a.WQ + hw + ka;
-            me.pad = 0;
+            const float aMl = g.a1 * cM;
             __syncwarp();
-            reinterpret_cast<float4*>(lp + lane)[0] = make_float4(me.PM0, me.Pm0, me.aM, me.am);
+            reinterpret_cast<float4*>(lp + lane)[0] = make_float4((float)(oMd + u0 * cMd), (float)(omd + u0 * cmd), aMl, g.a1 * cm);
             reinterpret_cast<float4*>(lp + lane)[1] =
-                make_float4(me.inv, __int_as_float(me.n), __int_as_float(me.soff), 0.f);
+                make_float4(1.0f / aMl, __int_as_float(kb - ka + 1), __int_as_float(th * a.WQ + hw + ka), 0.f);
             unsigned mask = __ballot_sync(0xffffffffu, hit);
             __syncwarp();
-            // lines of this batch one after the other; the samples of the NEXT line are copied into the other staging
-            // buffer (cp.async) while the current line is spread
-            int buf = 0;
-            auto stage = [&](int src, int bsel) {   // first kStg samples of line `src` -> stg[bsel]
-              const int n = lp[src].n;
-              const float2* row = Sp + lp[src].soff;
-              const unsigned dst = stg_addr + (unsigned)(bsel * kStg + 2 * lane) * 8u;
-              if (2 * lane < n) cp_async8(dst, row + 2 * lane);
-              if (2 * lane + 1 < n) cp_async8(dst + 8u, row + 2 * lane + 1);
-              cp_async_commit();
-            };
+            // lines of this batch one after the other.  Per line: (1) lane = sample evaluates what depends on the sample
+            // only (minor-axis weights, rows) into the warp's record; (2) lane = column walks the samples covering its
+            // column.  The samples of the NEXT line are fetched into a register while the current line is spread.
             int cur = -1;
+            float2 vreg = make_float2(0.f, 0.f);
             if (mask) {
               cur = __ffs(mask) - 1;
               mask &= mask - 1;
-              stage(cur, buf);
+              if (lane < lp[cur].n) vreg = __ldg(Sp + lp[cur].soff + lane);
             }
             while (cur >= 0) {
-              cp_async_wait_all();
-              __syncwarp();
+              const float4 q0 = reinterpret_cast<const float4*>(lp + cur)[0];
+              const float4 q1 = reinterpret_cast<const float4*>(lp + cur)[1];
+              const float PM0 = q0.x, Pm0 = q0.y, aM = q0.z, am = q0.w;
+              const int n = __float_as_int(q1.y), soff = __float_as_int(q1.z);
               int nxt = -1;
               if (mask) {
                 nxt = __ffs(mask) - 1;
                 mask &= mask - 1;
-                stage(nxt, buf ^ 1);
               }
-              const float4 q0 = reinterpret_cast<const float4*>(lp + cur)[0];
-              const float4 q1 = reinterpret_cast<const float4*>(lp + cur)[1];
-              const float PM0 = q0.x, Pm0 = q0.y, aM = q0.z, am = q0.w;
-              const int n = __float_as_int(q1.y);
               const float uA = (fL - 0.5f * W - PM0) * q1.x, uB = (fL + 0.5f * W - PM0) * q1.x;
               const int is = max(0, (int)ceilf(fminf(uA, uB) - 1e-3f));
               const int ie = min(n - 1, (int)floorf(fmaxf(uA, uB) + 1e-3f));
-              for (int seg = 0; seg < n; seg += kStg) {
-                if (seg > 0) {  // long runs (a1 < 2): later segments are fetched in place
-                  __syncwarp();
-                  const float2* row = Sp + __float_as_int(q1.z) + seg;
-                  stg[buf * kStg + 2 * lane] = seg + 2 * lane < n ? __ldg(row + 2 * lane) : make_float2(0.f, 0.f);
-                  stg[buf * kStg + 2 * lane + 1] = seg + 2 * lane + 1 < n ? __ldg(row + 2 * lane + 1) : make_float2(0.f, 0.f);
-                  __syncwarp();
+              float2 vnext = make_float2(0.f, 0.f);
+              for (int seg = 0; seg < n; seg += 32) {
+                if (seg > 0) vreg = seg + lane < n ? __ldg(Sp + soff + seg + lane) : make_float2(0.f, 0.f);  // long runs (a1 < 2)
+                __syncwarp();
+                {  // (1) lane = sample seg + lane
+                  const float Pm = fmaf((float)(seg + lane), am, Pm0);
+                  const float xm = Pm - 0.5f * W, rf = ceilf(xm);
+                  const int r0 = (int)rf;
+                  float2 eo[W / 2];
+                  const float dm = (xm - rf) + 0.5f;
+                  pieces(dm, eo);
+                  rec->v[lane] = vreg;
+#pragma unroll
+                  for (int j = 0; j < W / 2; ++j) {
+                    rec->wm[j][lane] = fmaf(dm, eo[j].y, eo[j].x);
+                    rec->wm[W - 1 - j][lane] = fmaf(-dm, eo[j].y, eo[j].x);
+                  }
+                  // bit j: row r0 + j is inside the tile (and the sample exists)
+                  const int lo = min(max(-r0, 0), W), hi = min(max(kTS - r0, 0), W);
+                  const unsigned rm = seg + lane < n ? ((1u << hi) - 1u) & ~((1u << lo) - 1u) : 0u;
+                  rec->pk[lane] = ((unsigned)r0 & 0xffu) | rm << 8;
                 }
-                const int ls = max(is, seg), cnt = min(ie, seg + kStg - 1) - ls + 1;
+                if (seg == 0 && nxt >= 0) vnext = lane < lp[nxt].n ? __ldg(Sp + lp[nxt].soff + lane) : make_float2(0.f, 0.f);
+                __syncwarp();
+                // (2) lane = column
+                const int ls = max(is, seg), cnt = min(ie, seg + 31) - ls + 1;
                 const int NI = __reduce_max_sync(0xffffffffu, cnt);
-                const float2* sv = stg + buf * kStg + (ls - seg);
+                if (NI <= 0) continue;
                 // software pipeline: the taps of pair i are loaded, the weights of pair i+1 are evaluated while those
                 // loads are in flight, then pair i is accumulated and stored
                 auto prep = [&](int i, float2& vw, float (&wm)[W], unsigned& addr, unsigned& rm) {
-                  const float fk = (float)(ls + i);
-                  const float2 P = __ffma2_rn(make_float2(fk, fk), make_float2(aM, am), make_float2(PM0, Pm0));
-                  const float xM = P.x - 0.5f * W, xm = P.y - 0.5f * W;
-                  const float cf = ceilf(xM), rf = ceilf(xm);
+                  const int k = min(ls - seg + i, 31);
+                  const float PM = fmaf((float)(ls + i), aM, PM0);
+                  const float xM = PM - 0.5f * W, cf = ceilf(xM);
                   const int j1 = lane - (int)cf;
-                  const int r0 = (int)rf;
                   const bool ok = i < cnt && (unsigned)j1 < (unsigned)W;
-                  const float2 v = sv[i < cnt ? i : 0];
-                  const float dM = (xM - cf) + 0.5f, dm = (xm - rf) + 0.5f;
-                  // E_j(d^2), O_j(d^2) of every half-tap j for both axes at once: .x major, .y minor
-                  const float2 d2 = __fmul2_rn(make_float2(dM, dm), make_float2(dM, dm));
-                  float2 e[W / 2], o[W / 2];
+                  const float2 v = rec->v[k];
+                  const unsigned pk = rec->pk[k];
 #pragma unroll
-                  for (int j = 0; j < W / 2; ++j) {
-                    e[j] = make_float2(cE[j][3], cE[j][3]);
-                    o[j] = make_float2(cO[j][3], cO[j][3]);
-#pragma unroll
-                    for (int q = 2; q >= 0; --q) {
-                      e[j] = __ffma2_rn(e[j], d2, make_float2(cE[j][q], cE[j][q]));
-                      o[j] = __ffma2_rn(o[j], d2, make_float2(cO[j][q], cO[j][q]));
-                    }
-                  }
-                  // major axis: this lane's tap j1 of the sample; taps j and W-1-j share E, O with opposite sign of d
+                  for (int j = 0; j < W; ++j) wm[j] = rec->wm[j][k];
+                  const float dM = (xM - cf) + 0.5f;
+                  float2 eo[W / 2];
+                  pieces(dM, eo);
+                  // this lane's tap j1 of the sample
                   const int jj = j1 < W / 2 ? j1 : W - 1 - j1;
-                  float eM = e[0].x, oM = o[0].x;
+                  float2 es = eo[0];
 #pragma unroll
                   for (int j = 1; j < W / 2; ++j) {
-                    eM = jj == j ? e[j].x : eM;
-                    oM = jj == j ? o[j].x : oM;
+                    es.x = jj == j ? eo[j].x : es.x;
+                    es.y = jj == j ? eo[j].y : es.y;
                   }
-                  const float wM = fmaf(j1 < W / 2 ? dM : -dM, oM, eM);
+                  const float wM = fmaf(j1 < W / 2 ? dM : -dM, es.y, es.x);
                   vw = make_float2(v.x * wM, v.y * wM);
-#pragma unroll
-                  for (int j = 0; j < W / 2; ++j) {
-                    wm[j] = fmaf(dm, o[j].y, e[j].y);
-                    wm[W - 1 - j] = fmaf(-dm, o[j].y, e[j].y);
-                  }
+                  const int r0 = (int)(signed char)(pk & 0xffu);
                   addr = mycol_addr + (unsigned)(r0 * (kTS * 8));
-                  // bit j: row r0 + j is inside the tile (and the pair exists)
-                  const int lo = min(max(-r0, 0), W), hi = min(max(kTS - r0, 0), W);
-                  rm = ok ? ((1u << hi) - 1u) & ~((1u << lo) - 1u) : 0u;
+                  rm = ok ? pk >> 8 : 0u;
                 };
-                float2 vw, nvw, c[W];
-                float wm[W], nwm[W];
-                unsigned addr, naddr, rm, nrm;
-                prep(0, vw, wm, addr, rm);
-                static_for<0, W>([&](auto J) {
-                  if (rm >> J.value & 1u) c[J.value] = lds_f2<j_off(J.value)>(addr);
-                });
-                for (int i = 0;;) {
-                  const bool last = i + 1 >= NI;
-                  if (!last) prep(i + 1, nvw, nwm, naddr, nrm);
-#pragma unroll
-                  for (int j = 0; j < W; ++j) {
-                    c[j].x = fmaf(vw.x, wm[j], c[j].x);
-                    c[j].y = fmaf(vw.y, wm[j], c[j].y);
-                  }
-                  static_for<0, W>([&](auto J) {
-                    if (rm >> J.value & 1u) sts_f2<j_off(J.value)>(addr, c[J.value]);
-                  });
-                  if (last) break;
-                  ++i;
-                  vw = nvw;
-#pragma unroll
-                  for (int j = 0; j < W; ++j) wm[j] = nwm[j];
-                  addr = naddr;
-                  rm = nrm;
+                if constexpr (kPipe) {
+                  float2 vw, nvw, c[W];
+                  float wm[W], nwm[W];
+                  unsigned addr, naddr, rm, nrm;
+                  prep(0, vw, wm, addr, rm);
                   static_for<0, W>([&](auto J) {
                     if (rm >> J.value & 1u) c[J.value] = lds_f2<j_off(J.value)>(addr);
                   });
+                  for (int i = 0;;) {
+                    const bool last = i + 1 >= NI;
+                    if (!last) prep(i + 1, nvw, nwm, naddr, nrm);
+#pragma unroll
+                    for (int j = 0; j < W; ++j) {
+                      c[j].x = fmaf(vw.x, wm[j], c[j].x);
+                      c[j].y = fmaf(vw.y, wm[j], c[j].y);
+                    }
+                    static_for<0, W>([&](auto J) {
+                      if (rm >> J.value & 1u) sts_f2<j_off(J.value)>(addr, c[J.value]);
+                    });
+                    if (last) break;
+                    ++i;
+                    vw = nvw;
+#pragma unroll
+                    for (int j = 0; j < W; ++j) wm[j] = nwm[j];
+                    addr = naddr;
+                    rm = nrm;
+                    static_for<0, W>([&](auto J) {
+                      if (rm >> J.value & 1u) c[J.value] = lds_f2<j_off(J.value)>(addr);
+                    });
+                  }
+                } else {
+#pragma unroll 1
+                  for (int i = 0; i < NI; ++i) {
+                    float2 vw, c[W];
+                    float wm[W];
+                    unsigned addr, rm;
+                    prep(i, vw, wm, addr, rm);
+                    static_for<0, W>([&](auto J) {
+                      if (rm >> J.value & 1u) c[J.value] = lds_f2<j_off(J.value)>(addr);
+                    });
+#pragma unroll
+                    for (int j = 0; j < W; ++j) {
+                      c[j].x = fmaf(vw.x, wm[j], c[j].x);
+                      c[j].y = fmaf(vw.y, wm[j], c[j].y);
+                    }
+                    static_for<0, W>([&](auto J) {
+                      if (rm >> J.value & 1u) sts_f2<j_off(J.value)>(addr, c[J.value]);
+                    });
+                  }
                 }
               }
               cur = nxt;
-              buf ^= 1;
+              vreg = vnext;
             }
             __syncwarp();
           }
