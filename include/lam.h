@@ -24,15 +24,21 @@
  *   vol   [nz][n][n]        float32, voxel (i3,i2,i1) <-> x = (i1-n/2, i2-n/2, i3-nz/2)
  *   dark, flat [h][w]       float32
  *
- * Pointers: proj / vol may be DEVICE pointers (in-core path; the plan's workspace must fit the device) or
- * HOST pointers (pinned or pageable; detected with cudaPointerGetAttributes): then the library streams chunks of
- * projections in and slabs of the volume out through its own pinned staging buffers on copy streams that overlap
- * the compute stream (Figs. 6-7).  The caller owns proj and vol; the plan owns every workspace.
+ * Pointers: proj / vol may be DEVICE pointers or HOST pointers (detected with cudaPointerGetAttributes), each on its
+ * own.  With a host pointer the library streams chunks of projections in / slabs of the volume out with
+ * cudaMemcpyAsync between the CALLER'S buffer and two plan-owned DEVICE staging buffers per direction, on plan-owned
+ * copy streams that overlap the compute stream (Figs. 6-7: three streams, 2 + 2 buffers).  There
+ * is no plan-owned pinned host staging: PINNED caller buffers (cudaHostAlloc / cudaHostRegister / torch pin_memory)
+ * give asynchronous, overlapped copies; PAGEABLE buffers are accepted and give the same result, but the CUDA runtime
+ * then stages every copy through its own bounce buffer and the copies do not overlap the kernels.  Every
+ * intermediate of the path stays in device memory: the plan's workspace must fit params.device_bytes whatever the
+ * pointer kinds are.  The caller owns proj and vol; the plan owns every workspace.
  *
  * All work of lam_backproject / lam_forward is enqueued on `cuda_stream` (a cudaStream_t, may be NULL = the
  * legacy default stream) and on plan-owned streams forked from / joined to it with events; the calls return
- * without synchronising when both pointers are device pointers.  With host pointers they return after the last
- * copy has completed.
+ * without synchronising when both pointers are device pointers.  With a host proj the call returns after the last
+ * host->device copy has completed (the caller may reuse proj), with a host vol after the last device->host copy
+ * (vol is complete on return).
  *
  * Errors: no exception or abort crosses this boundary.  Every function returns a lam_status; lam_last_error()
  * gives a plan-owned (or, for lam_create failures, thread-local) message.  There is NO CPU fallback: without a
@@ -53,7 +59,7 @@ typedef enum {
   LAM_OK = 0,
   LAM_EINVAL = 1,        /* bad argument (see lam_last_error)                              */
   LAM_ENOMEM_DEVICE = 2, /* workspace does not fit params.device_bytes / free device memory */
-  LAM_ENOMEM_HOST = 3,   /* pinned staging allocation failed                                */
+  LAM_ENOMEM_HOST = 3,   /* host allocation of the plan object failed                       */
   LAM_ECUDA = 4,         /* CUDA runtime error, or no device                                */
   LAM_EUNSUPPORTED = 5   /* valid request outside what this build implements                */
 } lam_status;
@@ -74,7 +80,7 @@ typedef struct {
   float center_v;      /* detector row hit by the ray through the origin; NaN -> h/2                        */
   float t_min;         /* transmission clamp before -log; 0 -> 1e-6                                         */
   size_t device_bytes; /* workspace budget; 0 -> 90 % of the free device memory at lam_create               */
-  int plane_batch;     /* k_v planes gridded + transformed per launch; 0 -> sized to stay L2-resident       */
+  int plane_batch;     /* k_v planes gridded + transformed per launch; 0 -> as many as fit 4 GB of fine grid  */
   int theta_chunk;     /* projections per filter/FFT launch (and per host->device copy); 0 -> auto          */
 } lam_params;
 
@@ -113,7 +119,7 @@ lam_status lam_set_profiling(lam_plan* plan, int on);
 
 /* Workspace facts of a plan, for benchmarks and tests:
  * info[0] device bytes allocated, info[1] k_v planes, info[2] plane batch, info[3] gridding work items (jobs),
- * info[4] 1 if the plan streams through the host (out-of-core), info[5] theta chunk,
+ * info[4] 1 if the last lam_backproject streamed through host pointers, info[5] theta chunk,
  * info[6] kernel launches of the last lam_backproject, info[7] pinned host bytes. */
 lam_status lam_plan_info(const lam_plan* plan, long long info[8]);
 

@@ -480,20 +480,41 @@ extern "C" void orc_fp_ray(const orc_geom* gp, const double* vol, double* proj) 
 //   kernel 1 (Gauss): kap(t) = exp(-t^2/(2 sg2)),  kaphat(s) = sqrt(2 pi sg2) exp(-2 pi^2 sg2 s^2)
 // shape = beta or sg2.  Taps m = ceil(t - W/2) + j, j = 0..W-1, stored periodically (reading Q7).
 // ---------------------------------------------------------------------------------------------
-static double kap(int kernel, int W, double shape, double t) {
+// Modified Bessel function I0 by its defining power series I0(x) = sum_k (x^2/4)^k / (k!)^2 (all terms positive, so
+// no cancellation; it replaces std::cyl_bessel_i in the tap loops, where that routine cost ~1 us per tap and made
+// the sliced path unusable at configs[2..4] sizes).  Pinned against scipy.special.i0 in tests/test_oracle_pins.py.
+static double i0_series(double x) {
+  static const struct InvK2 {   // 1/k^2, k = 1..255
+    double v[256];
+    InvK2() { v[0] = 0; for (int k = 1; k < 256; ++k) v[k] = 1.0 / ((double)k * (double)k); }
+  } inv;
+  double q = 0.25 * x * x, term = 1.0, sum = 1.0;
+  for (int k = 1; k < 256; ++k) {
+    term *= q * inv.v[k];
+    sum += term;
+    if (term < 1e-18 * sum) break;
+  }
+  return sum;
+}
+
+// kap with the constant I0(beta) handed in (it does not depend on t; the gridding loops evaluate it once)
+static double kap_n(int kernel, int W, double shape, double i0b, double t) {
   if (kernel == 0) {
     double r = 1.0 - (2.0 * t / W) * (2.0 * t / W);
     if (r < 0) return 0.0;
-    return std::cyl_bessel_i(0.0, shape * sqrt(r)) / std::cyl_bessel_i(0.0, shape);
+    return i0_series(shape * sqrt(r)) / i0b;
   }
   if (fabs(t) > 0.5 * W) return 0.0;
   return exp(-t * t / (2.0 * shape));
+}
+static double kap(int kernel, int W, double shape, double t) {
+  return kap_n(kernel, W, shape, kernel == 0 ? i0_series(shape) : 1.0, t);
 }
 
 static double kaphat(int kernel, int W, double shape, double s) {
   if (kernel == 0) {
     double q = shape * shape - (PI * W * s) * (PI * W * s);
-    double i0 = std::cyl_bessel_i(0.0, shape);
+    double i0 = i0_series(shape);
     if (q > 0) { double a = sqrt(q); return W / i0 * sinh(a) / a; }
     if (q < 0) { double a = sqrt(-q); return W / i0 * sin(a) / a; }
     return W / i0;
@@ -535,6 +556,9 @@ extern "C" int orc_fbp_gridded(const orc_geom* gp, const void* proj, int kernel,
   int M1 = (int)llround(sigma * n), M2 = M1, M3 = (int)llround(sigma * nz);
   std::vector<cd> G;
   try { G.assign((size_t)M1 * M2 * M3, cd(0, 0)); } catch (...) { return 1; }
+  const double i0b = kernel == 0 ? i0_series(shape) : 1.0;
+  std::vector<long long> B1((size_t)h * w), B2((size_t)h * w);
+  std::vector<double> K1((size_t)h * w * W), K2((size_t)h * w * W);
   std::vector<double> Hk(w), d((size_t)h * w);
   std::vector<cd> HD((size_t)h * w);
   make_filter(g, Hk.data());
@@ -542,6 +566,24 @@ extern "C" int orc_fbp_gridded(const orc_geom* gp, const void* proj, int kernel,
     load_proj(g, proj, th, d.data());
     spectrum(g, d.data(), Hk.data(), HD.data());
     double ct = cos(g.theta[th]), st = sin(g.theta[th]), cp = cos(g.phi), sp = sin(g.phi);
+    // taps and weights of every sample along xi1, xi2 (they depend on the sample only): one pass, rows shared out
+#pragma omp parallel for schedule(static)
+    for (int kv = -h / 2; kv < h - h / 2; ++kv) {
+      double fv = (double)kv / h;
+      for (int ku = -w / 2; ku < w - w / 2; ++ku) {
+        double fu = (double)ku / w;
+        double t1 = M1 * (fu * ct + fv * st * sp);   // Eq. 6 in fine-grid units
+        double t2 = M2 * (fu * st - fv * ct * sp);
+        size_t si = (size_t)(kv + h / 2) * w + ku + w / 2;
+        long long b1 = (long long)ceil(t1 - 0.5 * W), b2 = (long long)ceil(t2 - 0.5 * W);
+        B1[si] = b1;
+        B2[si] = b2;
+        for (int j = 0; j < W; ++j) {
+          K1[si * W + j] = kap_n(kernel, W, shape, i0b, t1 - (double)(b1 + j));
+          K2[si * W + j] = kap_n(kernel, W, shape, i0b, t2 - (double)(b2 + j));
+        }
+      }
+    }
     // each thread owns the fine planes m3 with (m3 mod nthreads) == tid, so no two threads write one cell
 #pragma omp parallel
     {
@@ -550,29 +592,23 @@ extern "C" int orc_fbp_gridded(const orc_geom* gp, const void* proj, int kernel,
 #else
       int tid = 0, nt = 1;
 #endif
-      std::vector<double> k1(W), k2(W), k3(W);
+      std::vector<double> k3(W);
       for (int kv = -h / 2; kv < h - h / 2; ++kv) {
         double fv = (double)kv / h;
         double t3 = M3 * (fv * cp);
         long long b3 = (long long)ceil(t3 - 0.5 * W);
-        for (int j = 0; j < W; ++j) k3[j] = kap(kernel, W, shape, t3 - (double)(b3 + j));
+        bool mine = false;
+        for (int j = 0; j < W; ++j) mine = mine || wrapi(b3 + j + M3 / 2, M3) % nt == tid;
+        if (!mine) continue;
+        for (int j = 0; j < W; ++j) k3[j] = kap_n(kernel, W, shape, i0b, t3 - (double)(b3 + j));
         for (int ku = -w / 2; ku < w - w / 2; ++ku) {
-          double fu = (double)ku / w;
-          double t1 = M1 * (fu * ct + fv * st * sp);   // Eq. 6 in fine-grid units
-          double t2 = M2 * (fu * st - fv * ct * sp);
-          long long b1 = (long long)ceil(t1 - 0.5 * W), b2 = (long long)ceil(t2 - 0.5 * W);
-          bool w1 = false;
-          cd val = HD[(size_t)(kv + h / 2) * w + ku + w / 2];
+          size_t si = (size_t)(kv + h / 2) * w + ku + w / 2;
+          long long b1 = B1[si], b2 = B2[si];
+          const double *k1 = &K1[si * W], *k2 = &K2[si * W];
+          cd val = HD[si];
           for (int j3 = 0; j3 < W; ++j3) {
             int m3 = wrapi(b3 + j3 + M3 / 2, M3);
             if (m3 % nt != tid) continue;
-            if (!w1) {
-              for (int j = 0; j < W; ++j) {
-                k1[j] = kap(kernel, W, shape, t1 - (double)(b1 + j));
-                k2[j] = kap(kernel, W, shape, t2 - (double)(b2 + j));
-              }
-              w1 = true;
-            }
             for (int j2 = 0; j2 < W; ++j2) {
               int m2 = wrapi(b2 + j2 + M2 / 2, M2);
               for (int j1 = 0; j1 < W; ++j1) {
@@ -611,6 +647,9 @@ extern "C" int orc_fbp_gridded_slice(const orc_geom* gp, const void* proj, int k
   int h = g.h, w = g.w, n = g.n, nz = g.nz;
   int M1 = (int)llround(sigma * n), M2 = M1;
   std::vector<cd> G((size_t)M1 * M2, cd(0, 0));
+  const double i0b = kernel == 0 ? i0_series(shape) : 1.0;
+  std::vector<long long> B1((size_t)h * w), B2((size_t)h * w);
+  std::vector<double> K1((size_t)h * w * W), K2((size_t)h * w * W);
   std::vector<double> Hk(w), d((size_t)h * w);
   std::vector<cd> HD((size_t)h * w);
   make_filter(g, Hk.data());
@@ -619,6 +658,25 @@ extern "C" int orc_fbp_gridded_slice(const orc_geom* gp, const void* proj, int k
     load_proj(g, proj, th, d.data());
     spectrum(g, d.data(), Hk.data(), HD.data());
     double ct = cos(g.theta[th]), st = sin(g.theta[th]), cp = cos(g.phi), sp = sin(g.phi);
+    // taps and weights of every sample (they depend on the sample only): one pass, rows shared out
+#pragma omp parallel for schedule(static)
+    for (int kv = -h / 2; kv < h - h / 2; ++kv) {
+      double fv = (double)kv / h;
+      for (int ku = -w / 2; ku < w - w / 2; ++ku) {
+        double fu = (double)ku / w;
+        double t1 = M1 * (fu * ct + fv * st * sp);
+        double t2 = M2 * (fu * st - fv * ct * sp);
+        size_t si = (size_t)(kv + h / 2) * w + ku + w / 2;
+        long long b1 = (long long)ceil(t1 - 0.5 * W), b2 = (long long)ceil(t2 - 0.5 * W);
+        B1[si] = b1;
+        B2[si] = b2;
+        for (int j = 0; j < W; ++j) {
+          K1[si * W + j] = kap_n(kernel, W, shape, i0b, t1 - (double)(b1 + j));
+          K2[si * W + j] = kap_n(kernel, W, shape, i0b, t2 - (double)(b2 + j));
+        }
+      }
+    }
+    // each thread owns the grid rows m2 with (m2 mod nthreads) == tid, so no two threads write one cell
 #pragma omp parallel
     {
 #ifdef _OPENMP
@@ -626,28 +684,18 @@ extern "C" int orc_fbp_gridded_slice(const orc_geom* gp, const void* proj, int k
 #else
       int tid = 0, nt = 1;
 #endif
-      std::vector<double> k1(W), k2(W);
       for (int kv = -h / 2; kv < h - h / 2; ++kv) {
         double fv = (double)kv / h;
         double a = 2.0 * PI * x3 * fv * cp;
         cd ph(cos(a), sin(a));
         for (int ku = -w / 2; ku < w - w / 2; ++ku) {
-          double fu = (double)ku / w;
-          double t1 = M1 * (fu * ct + fv * st * sp);
-          double t2 = M2 * (fu * st - fv * ct * sp);
-          long long b1 = (long long)ceil(t1 - 0.5 * W), b2 = (long long)ceil(t2 - 0.5 * W);
-          bool w1 = false;
-          cd val = HD[(size_t)(kv + h / 2) * w + ku + w / 2] * ph;
+          size_t si = (size_t)(kv + h / 2) * w + ku + w / 2;
+          long long b1 = B1[si], b2 = B2[si];
+          const double *k1 = &K1[si * W], *k2 = &K2[si * W];
+          cd val = HD[si] * ph;
           for (int j2 = 0; j2 < W; ++j2) {
             int m2 = wrapi(b2 + j2 + M2 / 2, M2);
             if (m2 % nt != tid) continue;
-            if (!w1) {
-              for (int j = 0; j < W; ++j) {
-                k1[j] = kap(kernel, W, shape, t1 - (double)(b1 + j));
-                k2[j] = kap(kernel, W, shape, t2 - (double)(b2 + j));
-              }
-              w1 = true;
-            }
             for (int j1 = 0; j1 < W; ++j1) {
               int m1 = wrapi(b1 + j1 + M1 / 2, M1);
               G[(size_t)m2 * M1 + m1] += val * (k1[j1] * k2[j2]);

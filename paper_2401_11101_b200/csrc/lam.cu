@@ -79,6 +79,7 @@ struct lam_plan {
   cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
   cudaEvent_t ev_in_ready[2] = {}, ev_in_free[2] = {}, ev_out_ready[2] = {}, ev_out_free[2] = {}, ev_fork = nullptr;
   bool host_path_ready = false;
+  bool last_call_host = false;   // the last lam_backproject streamed through host pointers
   // bookkeeping
   std::string err;
   int device = 0;
@@ -761,7 +762,9 @@ lam_status lam_backproject(lam_plan* p, const void* proj, float* vol, void* cuda
   CU(p, cudaGetLastError());
   if (g_launch_error != cudaSuccess) return fail(p, LAM_ECUDA, "kernel launch failed: %s", cudaGetErrorString(g_launch_error));
   p->stage_valid = p->profiling;
-  if (!vol_dev) CU(p, cudaStreamSynchronize(p->s_d2h));  // host results are valid on return
+  p->last_call_host = !proj_dev || !vol_dev;
+  if (!proj_dev) CU(p, cudaStreamSynchronize(p->s_h2d));  // the caller's host projections are consumed on return
+  if (!vol_dev) CU(p, cudaStreamSynchronize(p->s_d2h));   // host results are valid on return
   return LAM_OK;
 }
 
@@ -779,6 +782,7 @@ lam_status lam_forward(lam_plan* p, const float* vol, float* proj, void* cuda_st
   {
     ZTArgs za{vol, p->d_A, p->d_tw_M3, p->d_wz, p->d_bz, p->d_dx, p->d_dz, n, p->nz, NP, p->W};
     size_t sm = (size_t)kZCb * fft_tfast_pitch(p->M3, kZCb) * sizeof(float2);
+    if (sm > 220 * 1024) return fail(p, LAM_EUNSUPPORTED, "lam_forward: sigma*nz = %d does not fit the x3 stage's shared memory", p->M3);
     DISPATCH_LOG(p->logM3, zT(dim3(n / kZCb, n), sm, s, za));
     p->launches += 1;
   }
@@ -835,7 +839,7 @@ lam_status lam_plan_info(const lam_plan* p, long long info[8]) {
   info[1] = p->NP;
   info[2] = p->PB;
   info[3] = p->job_off.empty() ? 0 : p->job_off.back();
-  info[4] = 0;
+  info[4] = p->last_call_host ? 1 : 0;
   info[5] = p->TC;
   info[6] = p->launches;
   info[7] = (long long)p->pinned_bytes;

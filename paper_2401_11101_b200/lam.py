@@ -61,8 +61,8 @@ def lib():
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH):
-        build()
+    if not os.environ.get("LAM_LIB"):
+        build()             # rebuilds when a source is newer than the library (a stale .so is never loaded silently)
     L = C.CDLL(LIB_PATH)
     P = C.c_void_p
     L.lam_version.restype = C.c_char_p

@@ -1,13 +1,20 @@
 """GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (same plan parameters).
 
-The oracle cannot run a whole configs[2..4] scan (its exact path A costs N_theta (w h + nz h) complex MACs per
-x3-column after one double-precision 2-D FFT per projection).  The operator is linear in the projections, so the
-full-size plan (all N_theta angles in its geometry, all planes, all tiles, the default batches) is run on a scan in
-which only K angles carry data and the others hold zero line integrals; the exact answer is then the K-angle sum,
-which the oracle evaluates on sampled x3-columns.  Only the filter's quadrature weight pi cos(phi)/N_theta
-(reading Q3) differs between a K-angle and an N_theta-angle geometry: the oracle's K-angle result is scaled by
-K/N_theta, stated here and nowhere hidden.  Gate: rel L2 <= 1e-3 over the sampled columns (north_star).
+configs[1], [2]: the DENSE generated scan (every angle carries data, the arrays bench.py times) against the exact
+path A on 64 random x3-columns out to r = 0.45 n (the outer tiles, where the gridding work lists are sparse, are
+sampled as often as the centre), configs[1] also against two C' slices (Eq. 9 with the exact x3 phase).
+
+configs[3], [4] (uint16 + dark/flat): the oracle cannot follow 1800 / 3000 projections of 2048^2 / 2048 x 4096.
+The operator is linear in the line integrals, so the full-size plan (all N_theta angles in its geometry, every plane,
+tile and batch) runs on a scan in which K RANDOM angles carry the generated raw counts and the others hold raw = flat
+(a zero line integral, exactly, because the fixed-pattern fields are rounded to integers); the exact answer is the
+K-angle sum, which the oracle evaluates from the SAME uint16 + dark/flat arrays on 16 columns (path A) and two
+slices (C').  Only the filter's quadrature weight pi cos(phi)/N_theta (reading Q3) differs between a K-angle and an
+N_theta-angle geometry: the oracle's result is scaled by K/N_theta, stated here and nowhere hidden.  The angle subset
+changes from run to run (seed printed; LAM_TEST_SEED pins it); K/N_theta of the theta-dependent work lists carry data.
 """
+import os
+import time
 from dataclasses import replace
 
 import numpy as np
@@ -16,65 +23,108 @@ import torch
 
 from oracle import lam_oracle as O
 from paper_2401_11101_b200 import inputs, lam
+from gates import L2_NOISY, MAXABS_NOISY, NORTH_LARGE, check
 
 pytestmark = pytest.mark.gpu
-GATE_LARGE = 1e-3
-K = 4
-NCOLS = 8
+SEED = int(os.environ.get("LAM_TEST_SEED", str(int(time.time()) // 600)))
 
 
-def sparse_scan(cfg, device):
-    """Full-size input with data at K angles only.  Returns (proj tensor on `device`, sel, proj_sel numpy, dark, flat)."""
-    sel = np.linspace(0, cfg.ntheta, K, endpoint=False).astype(int) + 3
-    d = inputs.projections(replace(cfg, raw16=False, noise=0.0), device="cuda", theta=cfg.theta()[sel])["proj"]  # [K][h][w] f32
-    if cfg.raw16:
-        # integer-valued fields: raw = flat encodes a zero line integral exactly (PAPER.md:99 model)
-        dark = torch.full((cfg.h, cfg.w), 100.0)
-        flat = torch.full((cfg.h, cfg.w), 30000.0)
-        scale = 1.9 / float(d.max())
-        raw = torch.clamp(torch.round((30000.0 - 100.0) * torch.exp(-d * scale) + 100.0), 0, 65535).to(torch.int32).to(torch.uint16)
-        full = torch.full((cfg.ntheta, cfg.h, cfg.w), 30000, dtype=torch.uint16, device=device,
-                          **({"pin_memory": True} if device == "cpu" else {}))
-        for i, t in enumerate(sel):
-            full[int(t)].copy_(raw[i])
-        return full, sel, raw.cpu().numpy(), dark, flat
-    full = torch.zeros((cfg.ntheta, cfg.h, cfg.w), dtype=torch.float32, device=device)
-    full[torch.as_tensor(sel, device=device)] = d
-    return full, sel, d.cpu().numpy(), None, None
+def random_columns(cfg, ncols, rng):
+    """(i1, i2) uniform in the disc r <= 0.45 n (area-uniform: most of them in the outer half)."""
+    r = 0.45 * cfg.n * np.sqrt(rng.uniform(size=ncols))
+    a = rng.uniform(0, 2 * np.pi, size=ncols)
+    return np.stack([cfg.n // 2 + np.round(r * np.cos(a)), cfg.n // 2 + np.round(r * np.sin(a))], axis=1).astype(np.int32)
 
 
-def check_columns(cfg, vol, sel, proj_sel, dark, flat):
-    rng = np.random.default_rng(11 + cfg.n)
-    r = int(0.3 * cfg.n)
-    cols = (cfg.n // 2 + rng.integers(-r, r, size=(NCOLS, 2))).astype(np.int32)
-    g = O.Geometry(cfg.n, cfg.h, cfg.w, cfg.theta()[sel], cfg.phi, nz=cfg.nz,
-                   dark=None if dark is None else dark.numpy(), flat=None if flat is None else flat.numpy())
-    ref = O.fbp_nudft(g, proj_sel, cols=cols) * (K / cfg.ntheta)      # [ncols][nz]
-    got = np.stack([vol[:, c[1], c[0]].cpu().numpy().astype(np.float64) for c in cols])
-    err = float(np.linalg.norm(got - ref) / np.linalg.norm(ref))
-    assert np.isfinite(got).all()
-    assert err <= GATE_LARGE, err
-    return err
+def columns_of(vol, cols):
+    return np.stack([vol[:, int(c[1]), int(c[0])].cpu().numpy().astype(np.float64) for c in cols])
 
 
-@pytest.mark.parametrize("idx", [1, 2, 3])
-def test_full_size_sparse_angles_against_exact_columns(idx):
+@pytest.mark.parametrize("idx", [1, 2])
+def test_full_size_dense_scan_against_exact_columns(idx):
     cfg = inputs.config(idx)
+    rng = np.random.default_rng(SEED + idx)
+    d = inputs.projections(cfg, device="cuda")
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample)
+    vol = plan.backproject(d["proj"])
+    torch.cuda.synchronize()
+    info = plan.info()
+    plan.close()
+    proj = d["proj"].cpu().numpy()
+    del d
+    torch.cuda.empty_cache()
+    geom = O.Geometry(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz)
+    cols = random_columns(cfg, 64, rng)
+    ref = O.fbp_nudft(geom, proj, cols=cols)
+    e = check(columns_of(vol, cols), ref, L2_NOISY, MAXABS_NOISY, f"configs[{idx}] dense, 64 exact columns (seed {SEED})")
+    msg = f"configs[{idx}] dense full size: 64 exact columns rel L2 {e[0]:.3e} max-abs {e[1]:.3e}"
+    if idx == 1:
+        for i3 in rng.choice(cfg.nz, size=2, replace=False):
+            sl = O.fbp_gridded_slice(geom, proj, int(i3), W=cfg.width, sigma=cfg.oversample)
+            # error relative to the volume's RMS slice (a slice near the slab's edge is almost empty)
+            scale = float(vol.double().norm()) / np.sqrt(cfg.nz)
+            got = vol[int(i3)].cpu().numpy().astype(np.float64)
+            es = float(np.linalg.norm(got - sl)) / scale
+            assert es <= L2_NOISY, (int(i3), es)
+            msg += f", C' slice {int(i3)}: {es:.3e}"
+    print(msg, "plan =", info)
+
+
+def sparse_raw_scan(cfg, K, rng, device):
+    """Full-size uint16 scan with the generated counts at K random angles and raw = flat elsewhere."""
+    sel = np.sort(rng.choice(cfg.ntheta, size=K, replace=False))
+    dark, flat = inputs.detector_fields(cfg)
+    dark, flat = torch.round(dark), torch.round(flat)          # integer-valued: raw = flat is t = 1 exactly
+    sub = inputs.projections(replace(cfg, raw16=False, noise=0.0), device="cuda", theta=cfg.theta()[sel])["proj"]  # [K][h][w]
+    scale = cfg.dmax / float(sub.max())
+    gen = torch.Generator(device="cuda").manual_seed(int(rng.integers(1 << 31)))
+    cnt = (flat - dark).cuda()[None] * torch.exp(-sub * scale)
+    cnt = cnt + torch.sqrt(cnt) * torch.randn(cnt.shape, generator=gen, device="cuda")   # Poisson at these counts
+    raw = torch.clamp(torch.round(cnt + dark.cuda()[None]), 0, 65535).to(torch.int32).to(torch.uint16)
+    del sub, cnt
+    kw = {"pin_memory": True} if device == "cpu" else {}
+    full = torch.empty((cfg.ntheta, cfg.h, cfg.w), dtype=torch.uint16, device=device, **kw)
+    full.copy_(flat.to(torch.int32).to(torch.uint16)[None].expand_as(full))
+    for i, t in enumerate(sel):
+        full[int(t)].copy_(raw[i])
+    return full, sel, raw.cpu().numpy(), dark, flat
+
+
+def check_raw(cfg, vol, sel, raw_sel, dark, flat, rng, ncols=16, nslices=2):
+    K = len(sel)
+    geom = O.Geometry(cfg.n, cfg.h, cfg.w, cfg.theta()[sel], cfg.phi, nz=cfg.nz, dark=dark.numpy(), flat=flat.numpy())
+    cols = random_columns(cfg, ncols, rng)
+    ref = O.fbp_nudft(geom, raw_sel, cols=cols) * (K / cfg.ntheta)
+    e = check(columns_of(vol, cols), ref, L2_NOISY, MAXABS_NOISY, f"{cfg.name}: {ncols} exact columns (seed {SEED})")
+    msg = f"{ncols} exact columns rel L2 {e[0]:.3e} max-abs {e[1]:.3e}"
+    colrms = float(np.sqrt(np.mean(ref ** 2)))
+    for i3 in rng.choice(np.arange(cfg.nz // 4, 3 * cfg.nz // 4), size=nslices, replace=False):
+        sl = O.fbp_gridded_slice(geom, raw_sel, int(i3), W=cfg.width, sigma=cfg.oversample) * (K / cfg.ntheta)
+        got = vol[int(i3)].cpu().numpy().astype(np.float64)
+        es = float(np.sqrt(np.mean((got - sl) ** 2))) / max(colrms, float(np.sqrt(np.mean(sl ** 2))))
+        assert es <= NORTH_LARGE / 2, (int(i3), es)
+        msg += f", C' slice {int(i3)}: {es:.3e}"
+    return msg
+
+
+def test_config3_full_size_raw_uint16():
+    cfg = inputs.config(3)
     free, _ = torch.cuda.mem_get_info()
-    if idx == 3 and free < 120e9:
+    if free < 120e9:
         pytest.skip("configs[3] needs ~100 GB of device memory")
-    proj, sel, proj_sel, dark, flat = sparse_scan(cfg, "cuda")
-    plan = lam.Plan(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
-                    input="u16" if cfg.raw16 else "f32")
-    if cfg.raw16:
-        plan.set_darkflat(dark.cuda(), flat.cuda())
+    rng = np.random.default_rng(SEED + 3)
+    K = 64
+    proj, sel, raw_sel, dark, flat = sparse_raw_scan(cfg, K, rng, "cuda")
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample, input="u16")
+    plan.set_darkflat(dark.cuda(), flat.cuda())
     vol = plan.backproject(proj)
     torch.cuda.synchronize()
     info = plan.info()
     plan.close()
     del proj
-    err = check_columns(cfg, vol, sel, proj_sel, dark, flat)
-    print(f"configs[{idx}] full size: rel L2 on {NCOLS} exact columns = {err:.3e}, plan = {info}")
+    torch.cuda.empty_cache()
+    msg = check_raw(cfg, vol, sel, raw_sel, dark, flat, rng)
+    print(f"configs[3] full size, data at {K} of {cfg.ntheta} random angles ({100.0 * K / cfg.ntheta:.1f} % of theta): {msg}; plan = {info}")
 
 
 def test_config4_out_of_core_host_buffers():
@@ -84,23 +134,24 @@ def test_config4_out_of_core_host_buffers():
     cfg = inputs.config(4)
     free, _ = torch.cuda.mem_get_info()
     need_host = cfg.ntheta * cfg.h * cfg.w * 2 + cfg.voxels * 4
-    if free < 150e9 or psutil.virtual_memory().available < need_host + 20e9:
+    if free < 150e9 or psutil.virtual_memory().available < need_host + 30e9:
         pytest.skip("configs[4] needs ~145 GB of device memory and ~135 GB of host memory")
+    rng = np.random.default_rng(SEED + 4)
+    K = 32
     try:
-        proj, sel, proj_sel, dark, flat = sparse_scan(cfg, "cpu")
+        proj, sel, raw_sel, dark, flat = sparse_raw_scan(cfg, K, rng, "cpu")
         vol = torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, pin_memory=True)
     except RuntimeError as e:  # the host refuses to pin ~115 GB
         pytest.skip(f"cannot allocate the pinned host buffers of configs[4]: {e}")
-    plan = lam.Plan(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
-                    input="u16")
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample, input="u16")
     plan.set_darkflat(dark.cuda(), flat.cuda())
-    import time
     t0 = time.perf_counter()
     lam.lam_backproject(plan._plan, proj.data_ptr(), vol.data_ptr(), torch.cuda.current_stream().cuda_stream)
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     info = plan.info()
     plan.close()
-    err = check_columns(cfg, vol, sel, proj_sel, dark, flat)
-    print(f"configs[4] out-of-core: {dt:.2f} s wall ({cfg.voxels / dt / 1e9:.2f} GVoxel/s incl. PCIe), rel L2 on {NCOLS} "
-          f"exact columns = {err:.3e}, plan = {info}")
+    del proj
+    msg = check_raw(cfg, vol, sel, raw_sel, dark, flat, rng)
+    print(f"configs[4] out-of-core: {dt:.2f} s wall ({cfg.voxels / dt / 1e9:.2f} GVoxel/s incl. PCIe), data at {K} of "
+          f"{cfg.ntheta} random angles ({100.0 * K / cfg.ntheta:.1f} % of theta): {msg}; plan = {info}")

@@ -11,15 +11,23 @@ import torch
 from oracle import lam_oracle as O
 from paper_2401_11101_b200 import inputs, lam
 
+from gates import L2_CLEAN, L2_NOISY, MAXABS_CLEAN, MAXABS_NOISY, NORTH_LARGE, NORTH_TINY, check, rel
+
 pytestmark = pytest.mark.gpu
 
-GATE_TINY = 2e-4   # north_star: configs[0] against the exact oracle
-GATE_LARGE = 1e-3  # north_star: larger configs against the oracle's gridded path / exact columns
+GATE_TINY = NORTH_TINY    # north_star: configs[0] against the exact oracle (hard ceiling)
+GATE_LARGE = NORTH_LARGE  # north_star: larger configs (hard ceiling)
+assert L2_CLEAN <= GATE_TINY and L2_NOISY <= GATE_LARGE
 
 
-def rel(a, b):
-    a, b = np.asarray(a, dtype=np.float64), np.asarray(b, dtype=np.float64)
-    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+def tight(got, ref, what=""):
+    """noise-free fp32 inputs: rel L2 <= 5e-5 and max-abs <= 2e-4 max|ref| (tests/gates.py)"""
+    return check(got, ref, L2_CLEAN, MAXABS_CLEAN, what)
+
+
+def tight_noisy(got, ref, what=""):
+    """noisy / uint16 inputs: rel L2 <= 2e-4 and max-abs <= 1e-3 max|ref|"""
+    return check(got, ref, L2_NOISY, MAXABS_NOISY, what)
 
 
 def run_gpu(cfg, d, **kw):
@@ -51,8 +59,7 @@ def test_config0_tiny_against_exact_nudft_full_volume():
     vol, info = run_gpu(cfg, d)
     ref = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy())
     assert vol.shape == ref.shape == (cfg.nz, cfg.n, cfg.n)
-    assert np.isfinite(vol).all()
-    assert rel(vol, ref) <= GATE_TINY
+    print("configs[0] full volume vs exact NUDFT:", tight(vol, ref, "configs[0]"))
     assert info["launches"] > 0
 
 
@@ -62,7 +69,7 @@ def test_config0_other_filters(filt):
     d = inputs.projections(cfg)
     vol, _ = run_gpu(cfg, d, filter=filt)
     ref = O.fbp_nudft(geometry(cfg, d, filter=filt), d["proj"].numpy())
-    assert rel(vol, ref) <= GATE_TINY
+    tight(vol, ref, filt)
 
 
 def test_config0_gaussian_kernel_w8():
@@ -80,7 +87,7 @@ def test_config0_fractional_rotation_axis():
     cu, cv = cfg.w / 2 + 1.37, cfg.h / 2 - 0.61
     vol, _ = run_gpu(cfg, d, center_u=cu, center_v=cv)
     ref = O.fbp_nudft(geometry(cfg, d, cu=cu, cv=cv), d["proj"].numpy())
-    assert rel(vol, ref) <= GATE_TINY
+    tight(vol, ref, "fractional axis")
 
 
 def test_small_batches_give_the_same_answer():
@@ -101,12 +108,12 @@ def test_scaled_configs_against_gridded_oracle(idx, n):
     d = inputs.projections(cfg)
     vol, _ = run_gpu(cfg, d, plane_batch=24)
     ref = O.fbp_gridded(geometry(cfg, d), d["proj"].numpy())
-    assert rel(vol, ref) <= GATE_LARGE
+    e = tight_noisy(vol, ref, cfg.name)
     rng = np.random.default_rng(5)
     cols = rng.integers(0, cfg.n, size=(16, 2)).astype(np.int32)
     refA = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy(), cols=cols)     # [ncols][nz]
     got = np.stack([vol[:, c[1], c[0]] for c in cols])
-    assert rel(got, refA) <= GATE_LARGE
+    print(cfg.name, "vs C:", e, "vs A columns:", tight_noisy(got, refA, cfg.name + " columns"))
 
 
 def test_raw_uint16_darkflat_path():
@@ -116,7 +123,7 @@ def test_raw_uint16_darkflat_path():
     assert d["proj"].dtype == torch.uint16
     vol, _ = run_gpu(cfg, d)
     ref = O.fbp_gridded(geometry(cfg, d), d["proj"].numpy())
-    assert rel(vol, ref) <= GATE_LARGE
+    print("raw16:", tight_noisy(vol, ref, "raw16"))
 
 
 def test_wide_detector_nonsquare():
@@ -126,7 +133,7 @@ def test_wide_detector_nonsquare():
     assert cfg.w == 2 * cfg.h
     vol, _ = run_gpu(cfg, d)
     ref = O.fbp_gridded(geometry(cfg, d), d["proj"].numpy())
-    assert rel(vol, ref) <= GATE_LARGE
+    print("wide detector:", tight_noisy(vol, ref, "wide"))
 
 
 def test_phi_zero_is_slicewise_tomography():
@@ -137,7 +144,7 @@ def test_phi_zero_is_slicewise_tomography():
     d = inputs.projections(cfg)
     vol, _ = run_gpu(cfg, d)
     ref = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy())
-    assert rel(vol, ref) <= GATE_TINY
+    tight(vol, ref, "phi = 0")
 
 
 def test_repeat_calls_agree():
@@ -180,7 +187,7 @@ def test_long_transform_lengths_against_exact_columns(n, nz, h, w, nth):
     cols = (n // 2 + rng.integers(-r, r, size=(6, 2))).astype(np.int32)
     ref = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy(), cols=cols)
     got = np.stack([vol[:, c[1], c[0]] for c in cols])
-    assert rel(got, ref) <= GATE_TINY
+    tight(got, ref, f"fft {n} {h} {w}")
 
 
 def test_forward_against_exact_oracle():
@@ -199,7 +206,7 @@ def test_forward_against_exact_oracle():
     got = plan.forward(torch.from_numpy(f.astype(np.float32)).cuda()).cpu().numpy()
     plan.close()
     ref = O.forward_nudft(O.Geometry(n, h, w, theta, phi, nz=nz, filter="none"), f.astype(np.float32).astype(np.float64))
-    assert rel(got, ref) <= GATE_TINY
+    tight(got, ref, "lam_forward")
 
 
 @pytest.mark.parametrize("idx,n", [(2, 128), (4, 128)])
@@ -236,7 +243,7 @@ def test_very_few_angles(nth):
     d = inputs.projections(cfg)
     vol, _ = run_gpu(cfg, d)
     ref = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy())
-    assert rel(vol, ref) <= GATE_TINY
+    tight(vol, ref, "few angles")
 
 
 def test_arbitrary_unsorted_angles():
@@ -248,7 +255,7 @@ def test_arbitrary_unsorted_angles():
     d = inputs.projections(cfg, theta=theta)
     vol, _ = run_gpu(cfg, d)
     ref = O.fbp_nudft(geometry(cfg, d), d["proj"].numpy())
-    assert rel(vol, ref) <= GATE_TINY
+    tight(vol, ref, "unsorted angles")
 
 
 def test_width4_kernel_runs_and_is_as_accurate_as_its_oracle_twin():
@@ -269,5 +276,69 @@ def test_raw_counts_below_dark_are_clamped_like_the_oracle():
     d = dict(d, proj=raw)
     vol, _ = run_gpu(cfg, d)
     ref = O.fbp_gridded(geometry(cfg, d), raw.numpy())
-    assert np.isfinite(vol).all()
-    assert rel(vol, ref) <= GATE_LARGE
+    tight_noisy(vol, ref, "clamped counts")
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Full-band inputs: white noise puts energy into the out-of-band corners (periodic wrap, reading Q7) and into the
+# Nyquist rows / columns (symmetric split, reading Q8), which smooth blobs leave almost empty.
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,phi_deg,filt", [(32, 37.0, "ramp"), (32, 40.0, "none"), (64, 35.0, "ramp")])
+def test_white_noise_projections_against_exact_nudft(n, phi_deg, filt):
+    nth = 24 if n == 32 else 16
+    rng = np.random.default_rng(100 + n)
+    theta = 2 * np.pi * np.arange(nth) / nth + 0.05
+    phi = math.radians(phi_deg)
+    proj = rng.standard_normal((nth, n, n)).astype(np.float32)
+    plan = lam.Plan(n, n, n, theta, phi, filter=filt, plane_batch=5, theta_chunk=7)
+    vol = plan.backproject(torch.from_numpy(proj).cuda())
+    torch.cuda.synchronize()
+    plan.close()
+    geom = O.Geometry(n, n, n, theta, phi, filter=filt)
+    if n == 32:
+        ref = O.fbp_nudft(geom, proj)
+        got = vol.cpu().numpy()
+    else:
+        cols = rng.integers(0, n, size=(96, 2)).astype(np.int32)
+        ref = O.fbp_nudft(geom, proj, cols=cols)
+        got = np.stack([vol[:, int(c[1]), int(c[0])].cpu().numpy() for c in cols])
+    print(f"white noise n={n} phi={phi_deg} {filt}:", tight(got, ref, "white noise"))
+
+
+def test_forward_of_a_white_noise_volume_against_exact_nudft():
+    n, nz, nth = 32, 16, 10
+    rng = np.random.default_rng(77)
+    theta = 2 * np.pi * np.arange(nth) / nth + 0.2
+    phi = math.radians(38.0)
+    f = rng.standard_normal((nz, n, n)).astype(np.float32)
+    plan = lam.Plan(n, n, n, theta, phi, nz=nz, filter="none")
+    got = plan.forward(torch.from_numpy(f).cuda()).cpu().numpy()
+    plan.close()
+    ref = O.forward_nudft(O.Geometry(n, n, n, theta, phi, nz=nz, filter="none"), f.astype(np.float64))
+    print("forward, white-noise volume:", tight(got, ref, "lam_forward white noise"))
+
+
+@pytest.mark.parametrize("pinned", [True, False])
+def test_host_pointers_pinned_and_pageable(pinned):
+    """Host proj / vol (include/lam.h): several projection chunks in, several volume slabs out, same answer as the
+    device-pointer call."""
+    cfg = inputs.scaled(3, 128)
+    d = inputs.projections(cfg)
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, input="u16", theta_chunk=9, plane_batch=6)
+    plan.set_darkflat(d["dark"].cuda(), d["flat"].cuda())
+    ref = plan.backproject(d["proj"].cuda()).cpu()
+    hp = d["proj"].clone()
+    hv = torch.zeros((cfg.nz, cfg.n, cfg.n), dtype=torch.float32)
+    if pinned:
+        hp, hv = hp.pin_memory(), hv.pin_memory()
+    lam.lam_backproject(plan._plan, hp.data_ptr(), hv.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    # the call returns when the host volume is complete (header contract): no synchronisation here
+    assert rel(hv.numpy(), ref.numpy()) <= 2e-6
+    # mixed: host projections, device volume
+    dv = torch.empty_like(ref, device="cuda")
+    lam.lam_backproject(plan._plan, hp.data_ptr(), dv.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    hp.zero_()          # the call has consumed the host projections on return (header contract)
+    torch.cuda.synchronize()
+    assert rel(dv.cpu().numpy(), ref.numpy()) <= 2e-6
+    assert plan.info()["out_of_core"] == 1
+    plan.close()

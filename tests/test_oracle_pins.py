@@ -290,6 +290,17 @@ def test_Q7_out_of_band_samples_wrap():
     assert rel(O.fbp_gridded(geom, d, W=10), a) < 1e-7
 
 
+def test_kaiser_bessel_kernel_against_library_bessel():
+    """orc_kap evaluates I0 by its power series; scipy.special.i0 (a library routine on another algorithm) must
+    agree to rounding over the whole support, for several widths."""
+    from scipy.special import i0
+    for W, sigma in ((4, 2.0), (6, 2.0), (8, 2.0), (6, 1.5)):
+        beta = O.default_shape("kb", W, sigma)
+        for t in np.linspace(-W / 2, W / 2, 41):
+            want = i0(beta * math.sqrt(max(0.0, 1 - (2 * t / W) ** 2))) / i0(beta)
+            assert abs(O.kap("kb", W, beta, t) - want) <= 1e-13 * max(want, 1e-3)
+
+
 # ------------------------------------------------------------------ P9: path B ("Linerec", PAPER.md:111)
 def test_P9_direct_path_agrees_at_interpolation_level():
     """B differs from A only by the interpolation of the filtered projections (linear against trigonometric).
