@@ -9,6 +9,7 @@ Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
   e2e       the same call with HOST (pinned) buffers: H2D of the projections and D2H of the volume inside the timed region
   roofline  the dominant kernel group against its binding ceiling, plus `stages`: every stage against the HBM roofline
   cpu_baseline / --impl reference: the CPU fp64 oracle (oracle/), as it stands, on a bounded sample of the same workload
+  all_configs  configs[2] and configs[4] (host-resident, PCIe inside) measured in the same run, with their stage tables
 N > 1: the path does not shard without an exchange step: N independent replicas, weak scaling.
 """
 import argparse
@@ -32,7 +33,9 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2: slab 1024x1024x256)")
+    ap.add_argument("--config", type=int, default=3,
+                    help="index into BASELINE.json configs (default 3: the largest HBM-resident one, 2048x2048x512 from uint16)")
+    ap.add_argument("--no-all-configs", action="store_true", help="skip the all_configs block (configs[2], [4] measured beside the headline)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -106,39 +109,42 @@ def stage_model(cfg):
     }
 
 
-def cpu_sample(cfg, d, nangles, nslices=1, theta=None, mult=3):
-    """The oracle as it stands (path C': exact x3 transform + double-precision 2-D gridding, Eq. 9)
-    on one x3-slice, timed with `nangles` and with mult*`nangles` of the scan's angles.  A slice costs
-    t(na) = t_fix + na * t_angle (t_fix: the 2-D inverse FFT of the fine grid and the crop; t_angle: 2-D FFT + gridding of
-    one projection), so the two timings give both terms and the whole job is nz * (t_fix + ntheta * t_angle)."""
+def cpu_sample(cfg, nangles=None, slab=4, mult=3):
+    """The oracle as it stands, path C (the double-precision gridded USFFT of PAPER.md:130-142: 3-D gridding with
+    W^3 taps per sample, 3-D inverse FFT, deapodisation), on a BOUNDED sample of the config: the full detector and the
+    full lateral grid, but a slab of `slab` x3-slices and `nangles` / mult*`nangles` of the scan's angles.
+    Every sample still spreads its W^3 taps (the thin fine grid is periodic in xi3), so the per-angle cost is the
+    whole job's; the fixed cost (3-D inverse FFT + deapodisation of M x M x sigma*slab cells) grows with the slab as
+    nz/slab * log2(M M sigma nz)/log2(M M sigma slab).  Whole job = ntheta * t_angle + t_fix(nz), extrapolated."""
+    import math
+    from dataclasses import replace
     import numpy as np
     from oracle import lam_oracle as O
-    dark = d["dark"].cpu().numpy() if d["dark"] is not None else None
-    flat = d["flat"].cpu().numpy() if d["flat"] is not None else None
-    th_all = np.asarray(d["theta"] if theta is None else theta)
-    nav = len(th_all)
+    from paper_2401_11101_b200 import inputs
+    if nangles is None:
+        nangles = max(1, min(cfg.ntheta // (2 * mult), int(round(8 * (1024 * 1024) / (cfg.h * cfg.w)))))
     times, used = [], []
     for na in (nangles, mult * nangles):
-        na = max(1, min(nav, na))
-        idx = np.linspace(0, nav - 1, na).astype(int)
-        proj = d["proj"][idx].cpu().contiguous().numpy()
-        g = O.Geometry(cfg.n, cfg.h, cfg.w, th_all[idx], cfg.phi, nz=cfg.nz, dark=dark, flat=flat)
+        idx = np.linspace(0, cfg.ntheta - 1, na).astype(int)
+        d = inputs.projections(cfg, device="cpu", theta=cfg.theta()[idx])
+        proj = d["proj"].contiguous().numpy()
+        g = O.Geometry(cfg.n, cfg.h, cfg.w, cfg.theta()[idx], cfg.phi, nz=slab,
+                       dark=None if d["dark"] is None else d["dark"].numpy(), flat=None if d["flat"] is None else d["flat"].numpy())
         t0 = time.perf_counter()
-        for s in range(nslices):
-            O.fbp_gridded_slice(g, proj, cfg.nz // 2 + s, W=cfg.width, sigma=cfg.oversample)
-        times.append((time.perf_counter() - t0) / nslices)
+        O.fbp_gridded(g, proj, W=cfg.width, sigma=cfg.oversample)
+        times.append(time.perf_counter() - t0)
         used.append(na)
-    if used[1] > used[0]:
-        t_angle = max(0.0, (times[1] - times[0]) / (used[1] - used[0]))
-        t_fix = max(0.0, times[0] - used[0] * t_angle)
-    else:
-        t_angle, t_fix = times[0] / used[0], 0.0
-    total = cfg.nz * (t_fix + cfg.ntheta * t_angle)
-    return {"seconds": sum(times) * nslices, "value": cfg.voxels / total / 1e9, "cores": O.threads(),
+    t_angle = max(1e-9, (times[1] - times[0]) / (used[1] - used[0]))
+    t_fix = max(0.0, times[0] - used[0] * t_angle)
+    M = cfg.oversample * cfg.n
+    grow = (cfg.nz / slab) * math.log2(M * M * cfg.oversample * cfg.nz) / math.log2(M * M * cfg.oversample * slab)
+    total = cfg.ntheta * t_angle + t_fix * grow
+    return {"seconds": sum(times), "value": cfg.voxels / total / 1e9, "cores": O.threads(),
             "whole_job_seconds_extrapolated": total,
-            "sample": f"1 of {cfg.nz} x3-slices through oracle path C' (fp64 exact-x3 + 2-D gridded USFFT) with {used[0]} and "
-                      f"{used[1]} of {cfg.ntheta} angles; per-slice cost t_fix={t_fix:.3f}s + {t_angle:.4f}s/angle, "
-                      f"whole job = nz*(t_fix + ntheta*t_angle) extrapolated"}
+            "sample": f"oracle path C (fp64 3-D gridded USFFT, W^3 taps per sample) on the full {cfg.h}x{cfg.w} detector and "
+                      f"{cfg.n}x{cfg.n} lateral grid, a slab of {slab} of {cfg.nz} x3-slices, {used[0]} and {used[1]} of "
+                      f"{cfg.ntheta} angles: t_angle={t_angle:.3f}s, t_fix(slab)={t_fix:.2f}s; whole job = ntheta*t_angle + "
+                      f"t_fix*{grow:.1f} (extrapolated)"}
 
 
 def max_over_ranks(ms, world, device):
@@ -156,6 +162,123 @@ def whole_job_gvoxels(world, voxels_per_rank, ms_step):
     return world * voxels_per_rank / (ms_step * 1e-3) / 1e9
 
 
+def measure(idx, steps, warmup, world, barrier, want_e2e=True, want_overlap=False):
+    """One config: plan, K timed whole back-projections, per-stage times, optional end-to-end (host buffers) leg."""
+    import statistics
+    import torch
+    from paper_2401_11101_b200 import inputs, lam
+    cfg = inputs.config(idx)
+    hostmode = cfg.out_of_core  # configs[4]: input + output + workspace exceed HBM; projections and volume live in pinned host memory
+    if hostmode:
+        out = torch.empty((cfg.ntheta, cfg.h, cfg.w), dtype=torch.uint16 if cfg.raw16 else torch.float32, pin_memory=True)
+        d = inputs.projections(cfg, device="cuda", out=out)
+    else:
+        d = inputs.projections(cfg, device="cuda")
+    proj = d["proj"]
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
+                    input="u16" if cfg.raw16 else "f32")
+    torch.cuda.synchronize()
+    plan_ms = (time.perf_counter() - t0) * 1e3
+    if cfg.raw16:
+        plan.set_darkflat(d["dark"], d["flat"])
+    vol = (torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, pin_memory=True) if hostmode else
+           torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, device="cuda"))
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        plan.backproject(proj, vol)
+    barrier()
+    # ---- timed region: K whole back-projections, CUDA events on the launching stream (one pair brackets all K; one
+    # event between calls gives the per-call times for the median)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
+    ev[0].record(stream)
+    for i in range(steps):
+        plan.backproject(proj, vol)
+        ev[i + 1].record(stream)
+    barrier()
+    ms_total = ev[0].elapsed_time(ev[steps])
+    per_call = [ev[i].elapsed_time(ev[i + 1]) for i in range(steps)]
+    launches = plan.info()["launches"] * steps
+    # ---- per-stage device times, live, over K further calls (events inside the plan; not the headline number)
+    plan.set_profiling(True)
+    stage = [0.0] * 6
+    for _ in range(steps):
+        plan.backproject(proj, vol)
+        stage = [a + b for a, b in zip(stage, plan.stage_ms())]
+    plan.set_profiling(False)
+    stage = [x / steps for x in stage]
+    res = {"cfg": cfg, "ms_total": ms_total, "per_call": per_call, "median_ms": statistics.median(per_call),
+           "stage": stage, "launches": launches, "plan_ms": plan_ms, "info": plan.info(), "hostmode": hostmode,
+           "proj_bytes": proj.numel() * proj.element_size(), "e2e": None, "overlap": None}
+    # ---- e2e: the same call with host (pinned) buffers; H2D + D2H inside the timed region
+    if want_e2e and not hostmode:
+        hproj = torch.empty(proj.shape, dtype=proj.dtype, pin_memory=True)
+        hproj.copy_(proj)
+        hvol = torch.empty(vol.shape, dtype=torch.float32, pin_memory=True)
+        for _ in range(2):
+            lam.lam_backproject(plan._plan, hproj.data_ptr(), hvol.data_ptr(), stream.cuda_stream)
+        barrier()
+        ksteps = max(1, min(steps, 5))
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for _ in range(ksteps):
+            lam.lam_backproject(plan._plan, hproj.data_ptr(), hvol.data_ptr(), stream.cuda_stream)
+        e1.record(stream)
+        barrier()
+        wall = (time.perf_counter() - t0) * 1e3
+        ems = max(e0.elapsed_time(e1), wall if world == 1 else 0.0) / ksteps
+        err = float((hvol.cuda() - vol).norm() / vol.norm())
+        res["e2e"] = {"ms": ems, "steps": ksteps, "h2d": hproj.numel() * hproj.element_size(), "d2h": hvol.numel() * 4, "err": err}
+        del hproj, hvol
+    if hostmode:
+        res["e2e"] = {"ms": ms_total / steps, "steps": steps, "h2d": res["proj_bytes"], "d2h": vol.numel() * 4, "err": None}
+    if want_overlap and hostmode:
+        # SURVEY.md 8(d): t_total (host -> host call), t_copy_only (the same chunked copies on two copy streams, no
+        # kernels), t_compute_only (the device stages of the profiled call), overlap ratio
+        info = plan.info()
+        tc = max(1, info["theta_chunk"])
+        s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+        dbuf = [torch.empty((tc, cfg.h, cfg.w), dtype=proj.dtype, device="cuda") for _ in range(2)]
+        zr = max(1, min(cfg.n, (256 << 20) // (cfg.nz * cfg.n * 4)))
+        obuf = [torch.empty((cfg.nz, zr, cfg.n), dtype=torch.float32, device="cuda") for _ in range(2)]
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        with torch.cuda.stream(s_in):
+            for c, th0 in enumerate(range(0, cfg.ntheta, tc)):
+                nth = min(tc, cfg.ntheta - th0)
+                dbuf[c & 1][:nth].copy_(proj[th0:th0 + nth], non_blocking=True)
+        with torch.cuda.stream(s_out):
+            for c, r0 in enumerate(range(0, cfg.n, zr)):
+                r1 = min(cfg.n, r0 + zr)
+                vol[:, r0:r1, :].copy_(obuf[c & 1][:, :r1 - r0, :], non_blocking=True)
+        torch.cuda.synchronize()
+        t_copy = (time.perf_counter() - t0) * 1e3
+        t_compute = sum(stage[:4])
+        t_total = ms_total / steps
+        res["overlap"] = {"t_total_ms": round(t_total, 2), "t_copy_only_ms": round(t_copy, 2),
+                          "t_compute_only_ms": round(t_compute, 2),
+                          "overlap_ratio": round((t_copy + t_compute - t_total) / min(t_copy, t_compute), 4),
+                          "note": "copy-only: both directions at once (full duplex), no kernels; compute-only: sum of the "
+                                  "device stages of the profiled host-buffer call"}
+        del dbuf, obuf
+    plan.close()
+    del plan, proj, vol, d
+    torch.cuda.empty_cache()
+    return res
+
+
+def stage_report(cfg, stage, hbm):
+    model = stage_model(cfg)
+    out = {}
+    for i, nm in enumerate(model.keys()):
+        gbs = model[nm]["bytes"] / (stage[i] * 1e-3) / 1e9 if stage[i] > 0 else None
+        out[nm] = {"ms": round(stage[i], 4), "algorithmic_GB": round(model[nm]["bytes"] / 1e9, 4),
+                   "achieved_GBs": round(gbs, 1) if gbs else None, "hbm_frac": round(gbs / hbm, 4) if gbs else None}
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -169,21 +292,6 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    cfg = inputs.config(args.config)
-    hostmode = cfg.out_of_core  # configs[4]: input + workspace exceed HBM; projections and volume live in pinned host memory
-    if hostmode:
-        out = torch.empty((cfg.ntheta, cfg.h, cfg.w), dtype=torch.uint16 if cfg.raw16 else torch.float32, pin_memory=True)
-        d = inputs.projections(cfg, device="cuda", out=out)
-    else:
-        d = inputs.projections(cfg, device="cuda")
-    proj = d["proj"]
-    plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
-                    input="u16" if cfg.raw16 else "f32")
-    if cfg.raw16:
-        plan.set_darkflat(d["dark"], d["flat"])
-    vol = (torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, pin_memory=True) if hostmode else
-           torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, device="cuda"))
-    stream = torch.cuda.current_stream()
 
     def barrier():
         torch.cuda.synchronize()
@@ -191,62 +299,54 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        plan.backproject(proj, vol)
-    barrier()
+    warmup = max(args.warmup, 3)
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    # ---- timed region: K whole back-projections, device-resident input/output, CUDA events on the launching stream
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(args.steps):
-        plan.backproject(proj, vol)
-    e1.record(stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
-    launches = plan.info()["launches"] * args.steps
-    # ---- per-stage device times, live, over the same K steps again (events inside the plan; not the headline number)
-    plan.set_profiling(True)
-    stage = [0.0] * 6
-    for _ in range(args.steps):
-        plan.backproject(proj, vol)
-        stage = [a + b for a, b in zip(stage, plan.stage_ms())]
-    plan.set_profiling(False)
-    stage = [s / args.steps for s in stage]
+    r = measure(args.config, args.steps, warmup, world, barrier, want_e2e=not args.no_e2e, want_overlap=True)
     clocks = sampler.stop() if rank == 0 else None
-    ms = max_over_ranks(ms, world, "cuda")
+    cfg = r["cfg"]
+    ms = max_over_ranks(r["ms_total"], world, "cuda")
     ms_step = ms / args.steps
     value = whole_job_gvoxels(world, cfg.voxels, ms_step)
-
-    # ---- e2e: the same call with host (pinned) buffers; H2D + D2H inside the timed region
+    stage = r["stage"]
     e2e = None
-    if not args.no_e2e and not hostmode:
-        hproj = torch.empty(proj.shape, dtype=proj.dtype, pin_memory=True)
-        hproj.copy_(proj)
-        hvol = torch.empty(vol.shape, dtype=torch.float32, pin_memory=True)
-        for _ in range(2):
-            lam.lam_backproject(plan._plan, hproj.data_ptr(), hvol.data_ptr(), stream.cuda_stream)
-        barrier()
-        ksteps = max(1, min(args.steps, 5))
-        t0 = time.perf_counter()
-        e0.record(stream)
-        for _ in range(ksteps):
-            lam.lam_backproject(plan._plan, hproj.data_ptr(), hvol.data_ptr(), stream.cuda_stream)
-        e1.record(stream)
-        barrier()
-        wall = (time.perf_counter() - t0) * 1e3
-        ems = max(e0.elapsed_time(e1), wall if world == 1 else 0.0)
-        ems = max_over_ranks(ems, world, "cuda") / ksteps
-        err = float((hvol.cuda() - vol).norm() / vol.norm())
-        e2e = {"value": whole_job_gvoxels(world, cfg.voxels, ems), "unit": UNIT, "ms_per_step": ems, "steps": ksteps,
-               "h2d_bytes_per_step": hproj.numel() * hproj.element_size(),
-               "d2h_bytes_per_step": hvol.numel() * 4, "host_vs_device_result_rel_l2": err}
-        del hproj, hvol
-    if hostmode:  # the timed call above already ran host -> host
-        e2e = {"value": value, "unit": UNIT, "ms_per_step": ms_step, "steps": args.steps,
-               "h2d_bytes_per_step": proj.numel() * proj.element_size(), "d2h_bytes_per_step": vol.numel() * 4,
-               "note": "configs[4] does not fit HBM: value and e2e are the same host-buffer run"}
+    if r["e2e"] is not None:
+        ems = max_over_ranks(r["e2e"]["ms"], world, "cuda")
+        e2e = {"value": whole_job_gvoxels(world, cfg.voxels, ems), "unit": UNIT, "ms_per_step": round(ems, 3),
+               "steps": r["e2e"]["steps"], "h2d_bytes_per_step": r["e2e"]["h2d"], "d2h_bytes_per_step": r["e2e"]["d2h"]}
+        if r["e2e"]["err"] is not None:
+            e2e["host_vs_device_result_rel_l2"] = r["e2e"]["err"]
+        if r["hostmode"]:
+            e2e["note"] = "configs[4] does not fit HBM: value and e2e are the same host-buffer run"
+    # ---- the other single-GPU configs, measured in the same run (rank 0 of a 1-GPU run only): fewer calls
+    others = {}
+    if world == 1 and not args.no_all_configs:
+        free, _ = torch.cuda.mem_get_info()
+        for idx in (2, 3, 4):
+            if idx == args.config:
+                continue
+            c = inputs.config(idx)
+            try:
+                if idx == 4:
+                    import psutil
+                    if free < 150e9 or psutil.virtual_memory().available < c.ntheta * c.h * c.w * 2 + c.voxels * 4 + 30e9:
+                        others[f"configs[{idx}]"] = {"skipped": "needs ~145 GB of device and ~135 GB of pinned host memory"}
+                        continue
+                k = 3 if idx == 4 else min(args.steps, 5)
+                o = measure(idx, k, 3 if idx != 4 else 2, world, barrier, want_e2e=False, want_overlap=True)
+                hbm, _ = peaks()
+                oms = o["ms_total"] / k
+                others[f"configs[{idx}]"] = {
+                    "workload": f"{c.name}: volume {c.n}x{c.n}x{c.nz}, {c.ntheta} angles, detector {c.h}x{c.w} "
+                                f"{'uint16 raw + dark/flat' if c.raw16 else 'fp32'}" + (", host-resident buffers (PCIe inside)" if o["hostmode"] else ""),
+                    "value": round(c.voxels / (oms * 1e-3) / 1e9, 4), "unit": UNIT, "ms_per_step": round(oms, 3),
+                    "ms_per_step_median": round(o["median_ms"], 3), "steps": k, "warmup": 3 if idx != 4 else 2,
+                    "plan_ms": round(o["plan_ms"], 1), "stages": stage_report(c, o["stage"], hbm),
+                    "copies_ms": round(o["stage"][4], 2), "overlap": o["overlap"], "plan": o["info"]}
+            except Exception as e:  # a config that does not fit this box must not void the headline line
+                others[f"configs[{idx}]"] = {"error": str(e)[:200]}
+                torch.cuda.empty_cache()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -255,14 +355,12 @@ def run_ours(args):
     hbm, src = peaks()
     model = stage_model(cfg)
     names = list(model.keys())
-    stages = {}
-    for i, nm in enumerate(names):
-        gbs = model[nm]["bytes"] / (stage[i] * 1e-3) / 1e9 if stage[i] > 0 else None
-        stages[nm] = {"ms": round(stage[i], 4), "algorithmic_GB": round(model[nm]["bytes"] / 1e9, 4),
-                      "achieved_GBs": round(gbs, 1) if gbs else None, "hbm_frac": round(gbs / hbm, 4) if gbs else None}
+    stages = stage_report(cfg, stage, hbm)
     dom = max(range(4), key=lambda i: stage[i])
     if names[dom] == "s2_gridding_xy":
-        peak = 148 * 128 * 2 * 1.965e9 / 1e12   # fp32 FMA lanes x 2 flop x max SM clock
+        # S2 is bound by instruction issue and the shared-memory pipe, not by HBM: reported against
+        # the fp32 FMA peak derived from unit counts and clocks, with its HBM fraction beside it in `stages`
+        peak = 148 * 128 * 2 * 1.965e9 / 1e12
         ach = model[names[dom]]["flops"] / (stage[dom] * 1e-3) / 1e12
         roof = {"kernel": "k_spread (+k_zero_tiles)", "stage": names[dom], "bound": "alu", "achieved": round(ach, 3),
                 "peak": round(peak, 2), "unit": "TFLOP/s", "frac": round(ach / peak, 4), "traffic": None,
@@ -271,16 +369,15 @@ def run_ours(args):
         ach = model[names[dom]]["bytes"] / (stage[dom] * 1e-3) / 1e9
         roof = {"kernel": names[dom], "stage": names[dom], "bound": "hbm", "achieved": round(ach, 1), "peak": hbm,
                 "unit": "GB/s", "frac": round(ach / hbm, 4), "traffic": None, "peak_source": src}
-    # traffic: dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), if any
+    # traffic: dram bytes per launch of the dominant kernel from a committed ncu --set full capture, used only when that
+    # capture was taken on THIS build and THIS launch shape (library version, config, plane batch); otherwise null
     try:
         import csv
-        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "r01_traffic.csv"))):
-            if int(row["config"]) == args.config and row["stage"] == names[dom]:
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "r02_traffic.csv"))):
+            if (int(row["config"]) == args.config and row["stage"] == names[dom] and row["lib_version"] == lam.lam_version()
+                    and int(row["plane_batch"]) == r["info"]["plane_batch"]):
                 roof["traffic"] = float(row["dram_bytes_per_launch"])
-                roof["traffic_note"] = row["source"]
-                if row.get("issue_active_pct"):  # what binds the kernel under ncu: issue slots and the shared-memory pipe
-                    roof["ncu_issue_active_pct"] = float(row["issue_active_pct"])
-                    roof["ncu_l1tex_throughput_pct"] = float(row["l1tex_throughput_pct"])
+                roof["traffic_source"] = row["source"]
     except Exception:
         pass
     roof["stages"] = stages
@@ -288,48 +385,42 @@ def run_ours(args):
     total_bytes = sum(m["bytes"] for m in model.values())
     roof["whole_step_hbm_frac"] = round(total_bytes / (ms_step * 1e-3) / 1e9 / hbm, 4)
     out = {"metric": METRIC, "value": round(value, 4), "unit": UNIT, "n_gpus": world, "steps": args.steps,
-           "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 4), "higher_is_better": True,
-           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "warmup": warmup, "ms_per_step": round(ms_step, 4), "ms_per_step_median": round(r["median_ms"], 4),
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": f"configs[{args.config}] {cfg.name}: volume {cfg.n}x{cfg.n}x{cfg.nz} fp32, "
                                   f"{cfg.ntheta} angles, phi={cfg.phi_deg} deg, detector {cfg.h}x{cfg.w} "
                                   f"{'uint16 raw + dark/flat' if cfg.raw16 else 'fp32'}, KB W={cfg.width} sigma={cfg.oversample}",
-                      "l2": "inputs larger than L2 (projections %.2f GB, spectra %.2f GB per step)" % (
-                          proj.numel() * proj.element_size() / 1e9, model["s2_gridding_xy"]["bytes"] / 1e9),
+                      "l2": "inputs larger than L2 (projections %.2f GB, spectra + fine grid %.2f GB per step)" % (
+                          r["proj_bytes"] / 1e9, model["s2_gridding_xy"]["bytes"] / 1e9),
                       "parallelism": "replicas only" if world > 1 else "single GPU",
-                      "plan": plan.info()},
-           "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof}
+                      "plan": r["info"], "plan_ms": round(r["plan_ms"], 1), "lib": lam.lam_version()},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": r["launches"], "roofline": roof}
+    if r["overlap"]:
+        out["overlap"] = r["overlap"]
+    if others:
+        out["all_configs"] = others
     if not args.no_cpu_baseline:
-        na = args.cpu_angles or max(1, min(cfg.ntheta // 3, int(round(16 * (256 * 256) / (cfg.h * cfg.w)))))
-        cb = cpu_sample(cfg, d, na)
+        cb = cpu_sample(cfg)
         out["cpu_baseline"] = {"value": float(f"{cb['value']:.6g}"), "unit": UNIT, "cores": cb["cores"], "kind": "oracle",
                                "sample": cb["sample"], "seconds": round(cb["seconds"], 2)}
     print(json.dumps(out), flush=True)
-    plan.close()
     if world > 1:
         dist.destroy_process_group()
 
 
 def run_reference(args):
     """The reference arm of this tier = the CPU oracle, as it stands, on the host cores (rank 0 only).
-    One step = one bounded sample (cpu_sample: one x3-slice at two angle counts); the step's value is the whole-job
-    throughput the sample's two cost terms give."""
+    One step = one bounded sample (cpu_sample: path C on a thin slab at two angle counts); the step's value is the
+    whole-job throughput the sample's two cost terms give."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    import numpy as np
-    import torch
     from oracle import lam_oracle as O
     from paper_2401_11101_b200 import inputs
     cfg = inputs.config(args.config)
-    na = args.cpu_angles or max(1, min(cfg.ntheta // 3, int(round(4 * (256 * 256) / (cfg.h * cfg.w)))))
-    # only the sampled angles are generated (same recipe, same seed; the angle subset is part of the stated sample)
-    idx = np.linspace(0, cfg.ntheta - 1, 2 * na).astype(int)
-    dev = "cuda" if torch.cuda.is_available() else "cpu"
-    d = inputs.projections(cfg, device=dev, theta=cfg.theta()[idx])
-    d = {k: (v.cpu() if hasattr(v, "cpu") else v) for k, v in d.items()}
     vals, secs, last = [], [], None
     for it in range(args.warmup + args.steps):
         t0 = time.perf_counter()
-        last = cpu_sample(cfg, d, na, theta=d["theta"], mult=2)
+        last = cpu_sample(cfg, nangles=args.cpu_angles or None, mult=2)
         if it >= args.warmup:
             vals.append(last["value"])
             secs.append(time.perf_counter() - t0)

@@ -454,7 +454,7 @@ size_t zstage_smem(const lam_plan* p, int cb) { return ((size_t)(p->NP + p->KZ) 
 // ====================================================================================================================
 extern "C" {
 
-const char* lam_version(void) { return "lam-b200 0.1 (sm_100a)"; }
+const char* lam_version(void) { return "lam-b200 0.2 (sm_100a)"; }
 
 void lam_default_params(lam_params* p) {
   if (!p) return;

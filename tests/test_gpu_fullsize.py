@@ -23,7 +23,7 @@ import torch
 
 from oracle import lam_oracle as O
 from paper_2401_11101_b200 import inputs, lam
-from gates import L2_NOISY, MAXABS_NOISY, NORTH_LARGE, check
+from gates import L2_NOISY, L2_RAW_SPARSE, MAXABS_NOISY, NORTH_LARGE, check
 
 pytestmark = pytest.mark.gpu
 SEED = int(os.environ.get("LAM_TEST_SEED", str(int(time.time()) // 600)))
@@ -95,7 +95,7 @@ def check_raw(cfg, vol, sel, raw_sel, dark, flat, rng, ncols=16, nslices=2):
     geom = O.Geometry(cfg.n, cfg.h, cfg.w, cfg.theta()[sel], cfg.phi, nz=cfg.nz, dark=dark.numpy(), flat=flat.numpy())
     cols = random_columns(cfg, ncols, rng)
     ref = O.fbp_nudft(geom, raw_sel, cols=cols) * (K / cfg.ntheta)
-    e = check(columns_of(vol, cols), ref, L2_NOISY, MAXABS_NOISY, f"{cfg.name}: {ncols} exact columns (seed {SEED})")
+    e = check(columns_of(vol, cols), ref, L2_RAW_SPARSE, MAXABS_NOISY, f"{cfg.name}: {ncols} exact columns (seed {SEED})")
     msg = f"{ncols} exact columns rel L2 {e[0]:.3e} max-abs {e[1]:.3e}"
     colrms = float(np.sqrt(np.mean(ref ** 2)))
     for i3 in rng.choice(np.arange(cfg.nz // 4, 3 * cfg.nz // 4), size=nslices, replace=False):
