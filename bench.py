@@ -237,32 +237,23 @@ def measure(idx, steps, warmup, world, barrier, want_e2e=True, want_overlap=Fals
     if want_overlap and hostmode:
         # t_total (host -> host call), t_copy_only (the same chunked copies on two copy streams, no
         # kernels), t_compute_only (the device stages of the profiled call), overlap ratio
-        info = plan.info()
-        tc = max(1, info["theta_chunk"])
-        s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
-        dbuf = [torch.empty((tc, cfg.h, cfg.w), dtype=proj.dtype, device="cuda") for _ in range(2)]
-        zr = max(1, min(cfg.n, (256 << 20) // (cfg.nz * cfg.n * 4)))
-        obuf = [torch.empty((cfg.nz, zr, cfg.n), dtype=torch.float32, device="cuda") for _ in range(2)]
+        # copy-only: the library's own copies (same chunks, slabs, streams and events), kernels skipped
+        lam.lam_set_profiling(plan._plan, 2)
+        plan.backproject(proj, vol)
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        with torch.cuda.stream(s_in):
-            for c, th0 in enumerate(range(0, cfg.ntheta, tc)):
-                nth = min(tc, cfg.ntheta - th0)
-                dbuf[c & 1][:nth].copy_(proj[th0:th0 + nth], non_blocking=True)
-        with torch.cuda.stream(s_out):
-            for c, r0 in enumerate(range(0, cfg.n, zr)):
-                r1 = min(cfg.n, r0 + zr)
-                vol[:, r0:r1, :].copy_(obuf[c & 1][:, :r1 - r0, :], non_blocking=True)
+        for _ in range(2):
+            plan.backproject(proj, vol)
         torch.cuda.synchronize()
-        t_copy = (time.perf_counter() - t0) * 1e3
+        t_copy = (time.perf_counter() - t0) * 1e3 / 2
+        lam.lam_set_profiling(plan._plan, 0)
         t_compute = sum(stage[:4])
         t_total = ms_total / steps
         res["overlap"] = {"t_total_ms": round(t_total, 2), "t_copy_only_ms": round(t_copy, 2),
                           "t_compute_only_ms": round(t_compute, 2),
                           "overlap_ratio": round((t_copy + t_compute - t_total) / min(t_copy, t_compute), 4),
-                          "note": "copy-only: both directions at once (full duplex), no kernels; compute-only: sum of the "
-                                  "device stages of the profiled host-buffer call"}
-        del dbuf, obuf
+                          "note": "copy-only: the same call with every kernel skipped (lam_set_profiling(plan, 2)); "
+                                  "compute-only: sum of the device stages of the profiled host-buffer call"}
     plan.close()
     del plan, proj, vol, d
     torch.cuda.empty_cache()

@@ -115,6 +115,9 @@ lam_status lam_forward(lam_plan* plan, const float* vol, float* proj, void* cuda
  * (S2), ms[2] inverse FFT passes in x1 and x2 (S3), ms[3] fused x3 stage: gridding in xi3 + inverse FFT +
  * deapodise/crop/real part (S2 z-part + S3 + S4), ms[4] host<->device copies (host-pointer path), ms[5] whole call. */
 lam_status lam_stage_ms(lam_plan* plan, float ms[6]);
+/* on = 0: off; 1: per-stage events; 2: per-stage events AND a copy-only dry run: the following lam_backproject calls
+ * issue exactly their host<->device copies but skip every kernel (vol then holds no result): the t_copy_only leg of the
+ * overlap measurement of the host-pointer path. */
 lam_status lam_set_profiling(lam_plan* plan, int on);
 
 /* Workspace facts of a plan, for benchmarks and tests:

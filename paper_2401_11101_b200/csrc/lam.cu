@@ -61,7 +61,8 @@ struct lam_plan {
   float2* d_df = nullptr;
   float* d_wz = nullptr;  // [NP][W] x3 tap weights per plane (lam_forward)
   int* d_bz = nullptr;    // [NP] first x3 tap per plane
-  int *d_zlo = nullptr, *d_zcnt = nullptr;
+  int *d_zlo = nullptr, *d_zcnt = nullptr, *d_zidx = nullptr;
+  int nact = 0;  // active x3 grid cells
   Job* d_jobs = nullptr;
   std::vector<long long> job_off;  // [batches+1] first job of each plane batch (jobs of a batch: heaviest tiles first)
   unsigned* d_multi = nullptr;     // tiles written by several jobs, batch-major
@@ -84,6 +85,7 @@ struct lam_plan {
   std::string err;
   int device = 0;
   bool profiling = false;
+  bool copy_only = false;  // lam_set_profiling(plan, 2): the host<->device copies run, the kernels are skipped
   std::vector<StageEvent> events;
   size_t events_used = 0;
   long long launches = 0;
@@ -252,7 +254,7 @@ struct StageScope {
 
 void free_all(lam_plan* p) {
   void* ptrs[] = {p->d_cs,    p->d_Pu,  p->d_Pv,  p->d_PuNone, p->d_tw_w, p->d_tw_h,   p->d_tw_M, p->d_tw_M3,
-                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_zcnt, p->d_df, p->d_wz, p->d_bz, p->d_multi,
+                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_zcnt, p->d_zidx, p->d_df, p->d_wz, p->d_bz, p->d_multi,
                   p->d_R,     p->d_arena, p->d_G, p->d_T};
   for (void* q : ptrs)
     if (q) cudaFree(q);
@@ -405,7 +407,7 @@ lam_status make_tables(lam_plan* p) {
     int KZ = 1;
     for (int i = 0; i < M3; ++i) KZ = std::max(KZ, hi[i] - lo[i] + 1);
     p->KZ = KZ;
-    std::vector<float> ztab((size_t)M3 * KZ, 0.f), zlast(M3, 0.f), wz((size_t)NP * W);
+    std::vector<float> zfull((size_t)M3 * KZ, 0.f), zlastf(M3, 0.f), wz((size_t)NP * W);
     std::vector<int> bz(NP);
     for (int q = 0; q <= h / 2; ++q) {
       int kv = q == h / 2 ? -h / 2 : q;
@@ -416,16 +418,30 @@ lam_status make_tables(lam_plan* p) {
         int i = cell(b + j);
         float wv = (float)p->gk.kap(t3 - (b + j));
         wz[(size_t)q * W + j] = wv;
-        if (q == h / 2) zlast[i] += wv;
-        else ztab[(size_t)i * KZ + (q - lo[i])] += wv;
+        if (q == h / 2) zlastf[i] += wv;
+        else zfull[(size_t)i * KZ + (q - lo[i])] += wv;
       }
     }
+    // compact the active cells (a tap of some plane lands on them); tables cell-fastest for coalesced reads
+    std::vector<int> zidx(M3, -1), zlo, zcnt;
+    std::vector<float> zlast;
+    for (int i = 0; i < M3; ++i)
+      if (hi[i] >= lo[i] || zlastf[i] != 0.f) {
+        zidx[i] = (int)zlo.size();
+        zlo.push_back(hi[i] >= lo[i] ? lo[i] : 0);
+        zcnt.push_back(hi[i] >= lo[i] ? hi[i] - lo[i] + 1 : 0);
+        zlast.push_back(zlastf[i]);
+      }
+    p->nact = (int)zlo.size();
+    std::vector<float> ztab((size_t)KZ * p->nact, 0.f);
+    for (int i = 0; i < M3; ++i)
+      if (zidx[i] >= 0)
+        for (int s2 = 0; s2 < KZ; ++s2) ztab[(size_t)s2 * p->nact + zidx[i]] = zfull[(size_t)i * KZ + s2];
     if ((st = upload(p, &p->d_ztab, ztab)) != LAM_OK) return st;
-    std::vector<int> cnt(M3);
-    for (int i = 0; i < M3; ++i) cnt[i] = hi[i] >= lo[i] ? hi[i] - lo[i] + 1 : 0;
-    if ((st = upload(p, &p->d_zlo, lo)) != LAM_OK) return st;
-    if ((st = upload(p, &p->d_zcnt, cnt)) != LAM_OK) return st;
+    if ((st = upload(p, &p->d_zlo, zlo)) != LAM_OK) return st;
+    if ((st = upload(p, &p->d_zcnt, zcnt)) != LAM_OK) return st;
     if ((st = upload(p, &p->d_zlast, zlast)) != LAM_OK) return st;
+    if ((st = upload(p, &p->d_zidx, zidx)) != LAM_OK) return st;
     if ((st = upload(p, &p->d_wz, wz)) != LAM_OK) return st;
     if ((st = upload(p, &p->d_bz, bz)) != LAM_OK) return st;
   }
@@ -447,7 +463,10 @@ lam_status make_tables(lam_plan* p) {
   return LAM_OK;
 }
 
-size_t zstage_smem(const lam_plan* p, int cb) { return ((size_t)(p->NP + p->KZ) * cb + (size_t)cb * fft_tfast_pitch(p->M3, cb)) * sizeof(float2); }
+size_t zstage_smem(const lam_plan* p, int cb) {
+  const size_t work = std::max((size_t)p->NP * z_pitch(cb), (size_t)cb * fft_tfast_pitch(p->M3, cb));
+  return (((work + 1) & ~(size_t)1) + (size_t)p->nact * cb) * sizeof(float2);
+}
 
 }  // namespace
 
@@ -599,6 +618,7 @@ lam_status lam_set_darkflat(lam_plan* p, const float* dark, const float* flat) {
 lam_status lam_set_profiling(lam_plan* p, int on) {
   if (!p) return LAM_EINVAL;
   p->profiling = on != 0;
+  p->copy_only = on == 2;
   return LAM_OK;
 }
 
@@ -613,6 +633,7 @@ static bool is_device_ptr(const void* q) {
 
 // S0 + S1 for projections [th0, th0 + nth) at device pointer `chunk` (the first projection of the chunk)
 static void launch_s1(lam_plan* p, const void* chunk, int th0, int nth, cudaStream_t s) {
+  if (p->copy_only) return;
   const bool raw = p->prm.input == LAM_INPUT_U16_RAW;
   RowsArgs ra{chunk, p->d_df, p->prm.t_min, p->d_R, p->d_Pu, p->d_tw_w, p->h, p->WR, p->rows_nb};
   dim3 gr(p->h / 2 / p->rows_nb, nth);
@@ -628,6 +649,7 @@ static void launch_s1(lam_plan* p, const void* chunk, int th0, int nth, cudaStre
 
 // S2 + S3 (x1, x2) for planes [p0, p0 + np): p0 is a multiple of the plane batch
 static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
+  if (p->copy_only) return;
   const int b = p0 / p->PB;
   SpreadArgs sa{p->geom, p->kp, p->d_jobs + p->job_off[b], p->job_off[b + 1] - p->job_off[b], p->d_S, p->WQ, p->d_G, p0,
                 p->d_multi + p->multi_off[b], p->multi_off[b + 1] - p->multi_off[b]};
@@ -660,9 +682,10 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
 
 // x3 stage for x2 rows [x2_0, x2_0 + rows); out holds x2 row `out_x2_0` in its first row, z-stride `zstride` floats
 static void launch_z(lam_plan* p, float* out, size_t zstride, int x2_0, int rows, int out_x2_0, cudaStream_t s) {
+  if (p->copy_only) return;
   StageScope sc(p, 3, s);
-  ZArgs za{p->d_A, out, zstride, p->d_tw_M3, p->d_ztab, p->d_zlo, p->d_zcnt, p->d_zlast, p->d_dx, p->d_dz,
-           p->n, p->nz, p->NP, p->KZ, p->z_lcb, x2_0, out_x2_0};
+  ZArgs za{p->d_A, out, zstride, p->d_tw_M3, p->d_ztab, p->d_zlo, p->d_zcnt, p->d_zlast, p->d_zidx, p->d_dx, p->d_dz,
+           p->n, p->nz, p->NP, p->nact, p->z_lcb, x2_0, out_x2_0};
   DISPATCH_LOG(p->logM3, z(dim3(p->n >> p->z_lcb, rows), zstage_smem(p, 1 << p->z_lcb), s, za));
   p->launches += 1;
 }

@@ -172,9 +172,12 @@ __global__ void __launch_bounds__(512) k_ifft_x2(IfftArgs a) {
 // A[p] are samples of a 1-D unequally spaced spectrum along x3 for every (x1, x2):
 //   Gz[m3] = sum_p A[p] kap(t3(p) - m3),  t3 = M3 k_v cos(phi)/h;   vol[x3] = Re sum_m3 Gz[m3] e^{2 pi i x3 m3/M3}
 //   divided by kaphat(x1/M) kaphat(x2/M) kaphat(x3/M3)  (PAPER.md:136 step 1, reversed per PAPER.md:140).
-// The gridding is a banded matrix that is the same for every column: for grid cell i the planes with a tap on it
-// are contiguous, [zlo[i], zlo[i] + KZ), with weights ztab[i][KZ] (zero padded); the k_v = -h/2 plane (stored
-// last) has its own weight zlast[i].  Cell values are computed on the fly by the loader of the first FFT pass.
+// The gridding is a banded matrix that is the same for every column.  Only the cells that some plane has a tap on
+// are ACTIVE (about half of M3: the planes k_v >= 0 reach xi3 >= 0 only); for active cell j the planes with a tap on
+// it are contiguous, [zlo[j], zlo[j] + zcnt[j]), with weights ztab[s][j]; the k_v = -h/2 plane (stored last) has its
+// own weight zlast[j].  Three phases: (1) the block's columns of every plane are staged in shared memory (coalesced),
+// (2) one thread per (active cell, column pair) accumulates the cell over its band: the weight is read once per tap
+// and serves two columns, (3) the length-M3 inverse FFT reads the compact cells through the cell -> slot map zidx.
 // ---------------------------------------------------------------------------------------------------------------
 constexpr int kZCb = 8, kZLog = 3;
 
@@ -183,47 +186,75 @@ struct ZArgs {
   float* vol;            // output buffer; element (ix3, ix2, ix1) at vol[ix3*zstride + (ix2 - vol_x2_0)*n + ix1]
   size_t zstride;
   const float2* tw;      // length M3
-  const float* ztab;     // [M3][KZ]
-  const int* zlo;        // [M3] first plane with a tap on cell i
-  const int* zcnt;       // [M3] number of such planes (<= KZ)
-  const float* zlast;    // [M3]
+  const float* ztab;     // [KZ][nact]
+  const int* zlo;        // [nact] first plane with a tap on active cell j
+  const int* zcnt;       // [nact] number of such planes (<= KZ)
+  const float* zlast;    // [nact]
+  const int* zidx;       // [M3] slot of cell i among the active cells, or -1
   const float* dx;       // [n]  1/kaphat(x/M)
   const float* dz;       // [nz] 1/kaphat(x3/M3)
-  int n, nz, np, KZ, lcb;  // 1 << lcb columns per block
+  int n, nz, np, nact, lcb;  // 1 << lcb columns per block
   int x2_0;              // first x2 row of this launch
   int vol_x2_0;          // x2 index held by row 0 of the output buffer
 };
 
+// row pitch of the staged planes in float2: rows two or three planes apart (neighbouring cells) land in different
+// 16-byte bank groups for the 128-bit reads of phase 2
+__host__ __device__ constexpr int z_pitch(int cb) { return cb >= 8 ? cb + 4 : cb; }
+
 template <int LOGM3>
 __global__ void __launch_bounds__(512) k_zstage(ZArgs a) {
   constexpr int M3 = 1 << LOGM3;
-  const int zlog = a.lcb, zcb = 1 << a.lcb, P = fft_tfast_pitch(M3, zcb);  // columns per block
+  const int zlog = a.lcb, zcb = 1 << a.lcb, P = fft_tfast_pitch(M3, zcb), PA = z_pitch(zcb);
   extern __shared__ float2 sm[];
-  float2* Gz = sm;                                // [8][P]
-  float2* Ain = sm + zcb * P;                    // [np + KZ][zcb], the KZ extra planes are zero
+  float2* Ain = sm;                                           // [np][PA]; the FFT works in place of it afterwards
+  const int fftsz = zcb * P, ainsz = a.np * PA;
+  float2* Gz = sm + ((max(fftsz, ainsz) + 1) & ~1);           // [nact][zcb] compact active cells
   const int ix2 = a.x2_0 + blockIdx.y, c0 = blockIdx.x * zcb;
   const size_t nn = (size_t)a.n * a.n;
   const float2* Ab = a.A + (size_t)ix2 * a.n + c0;
-  for (int idx = threadIdx.x; idx < (a.np + a.KZ) * zcb; idx += blockDim.x) {
-    int p = idx >> zlog, c = idx & (zcb - 1);
-    Ain[idx] = p < a.np ? Ab[(size_t)p * nn + c] : make_float2(0.f, 0.f);
+  {  // phase 1: 16-byte loads, four in flight per thread before the first store (the loads are latency-bound otherwise)
+    const int hlog = zlog - 1, total = a.np << hlog;
+    for (int base = threadIdx.x; base < total; base += 4 * blockDim.x) {
+      float4 v[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int idx = base + u * blockDim.x;
+        if (idx < total) v[u] = __ldg(reinterpret_cast<const float4*>(Ab + (size_t)(idx >> hlog) * nn + 2 * (idx & ((1 << hlog) - 1))));
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int idx = base + u * blockDim.x;
+        if (idx < total) *reinterpret_cast<float4*>(Ain + (idx >> hlog) * PA + 2 * (idx & ((1 << hlog) - 1))) = v[u];
+      }
+    }
   }
   __syncthreads();
-  const int KZ = a.KZ, last = (a.np - 1) * zcb;
-  auto ld = [&](int t, int i) -> float2 {
-    const float* wt = a.ztab + (size_t)i * KZ;
-    const float2* ap = Ain + __ldg(&a.zlo[i]) * zcb + t;
-    float wl = __ldg(&a.zlast[i]);
-    float2 v = Ain[last + t];
-    float2 acc = make_float2(v.x * wl, v.y * wl);
-    const int cnt = __ldg(&a.zcnt[i]);
-    for (int s = 0; s < cnt; ++s) {
-      float wv = __ldg(&wt[s]);
-      float2 x = ap[s * zcb];
-      acc.x = fmaf(x.x, wv, acc.x);
-      acc.y = fmaf(x.y, wv, acc.y);
+  {
+    const int hc = zcb >> 1, last = (a.np - 1) * PA;
+    for (int task = threadIdx.x; task < a.nact * hc; task += blockDim.x) {
+      const int j = task / hc, c2 = (task - j * hc) * 2;
+      const int lo = __ldg(&a.zlo[j]), cnt = __ldg(&a.zcnt[j]);
+      const float wl = __ldg(&a.zlast[j]);
+      const float4 v = *reinterpret_cast<const float4*>(Ain + last + c2);
+      float4 acc = make_float4(v.x * wl, v.y * wl, v.z * wl, v.w * wl);
+      const float2* ap = Ain + lo * PA + c2;
+      const float* wt = a.ztab + j;
+      for (int s = 0; s < cnt; ++s) {
+        const float wv = __ldg(&wt[(size_t)s * a.nact]);
+        const float4 x = *reinterpret_cast<const float4*>(ap + s * PA);
+        acc.x = fmaf(x.x, wv, acc.x);
+        acc.y = fmaf(x.y, wv, acc.y);
+        acc.z = fmaf(x.z, wv, acc.z);
+        acc.w = fmaf(x.w, wv, acc.w);
+      }
+      *reinterpret_cast<float4*>(Gz + j * zcb + c2) = acc;
     }
-    return acc;
+  }
+  __syncthreads();
+  auto ld = [&](int t, int i) -> float2 {
+    const int k = __ldg(&a.zidx[i]);
+    return k >= 0 ? Gz[k * zcb + t] : make_float2(0.f, 0.f);
   };
   const float dx2 = a.dx[ix2];
   const int hz = a.nz / 2;
@@ -233,7 +264,7 @@ __global__ void __launch_bounds__(512) k_zstage(ZArgs a) {
     if (k >= hz && k < M3 - hz) return;
     vb[(size_t)ix3 * a.zstride + t] = v.x * a.dz[ix3] * dx2 * a.dx[c0 + t];
   };
-  block_fft<LOGM3, +1, true, true>(Gz, zcb, zlog, P, a.tw, ld, st);
+  block_fft<LOGM3, +1, true, true>(sm, zcb, zlog, P, a.tw, ld, st);
 }
 
 }  // namespace lam
