@@ -51,6 +51,8 @@ typedef struct {
   const float* dark;    // h*w, dtype 2 only
   const float* flat;    // h*w, dtype 2 only
   double tmin;          // transmission clamp for -log
+  int pad;              // rows edge-extended to pad*w samples before the filter (reading Q11b); 0 or 1: none
+  double alpha;         // 2-D spectral multiplier 1/(1 + alpha ((k_u/w)^2 + (k_v/h)^2)) on the projections; 0: none
 } orc_geom;
 }
 
@@ -150,7 +152,7 @@ extern "C" void orc_prep(const orc_geom* g, const void* proj, int th, double* ou
 // Output Hk[k_u + w/2], real.
 // ---------------------------------------------------------------------------------------------
 static double ramp_kernel(int filter, int j) {
-  if (filter == 1) {
+  if (filter == 1 || filter == 3) {
     if (j == 0) return 0.25;
     if (j % 2 == 0) return 0.0;
     return -1.0 / (PI * PI * (double)j * (double)j);
@@ -158,19 +160,32 @@ static double ramp_kernel(int filter, int j) {
   return -2.0 / (PI * PI * (4.0 * (double)j * (double)j - 1.0));
 }
 
-static void make_filter(const orc_geom& g, double* Hk) {
-  int w = g.w;
-  if (g.filter == 0) { for (int i = 0; i < w; ++i) Hk[i] = 1.0; return; }
+// Parzen (de la Vallee Poussin) window, "low pass filters (shepp-logan, parzen)"; reading Q15: the ramp
+// response times P(x), x = |k_u| / (len/2) in [0, 1] (1 = Nyquist):
+//   P(x) = 1 - 6 x^2 + 6 x^3  (x <= 1/2),   2 (1 - x)^3  (1/2 < x <= 1).
+static double parzen(double x) {
+  x = fabs(x);
+  if (x <= 0.5) return 1.0 - 6.0 * x * x + 6.0 * x * x * x;
+  if (x <= 1.0) return 2.0 * (1.0 - x) * (1.0 - x) * (1.0 - x);
+  return 0.0;
+}
+
+// filter response for rows of `len` samples (len = w, or pad*w for padded rows): Hk[k + len/2], k in [-len/2, len/2)
+static void make_filter_len(const orc_geom& g, int len, double* Hk) {
+  if (g.filter == 0) { for (int i = 0; i < len; ++i) Hk[i] = 1.0; return; }
   double scale = PI * cos(g.phi) / g.ntheta;
-  for (int ku = -w / 2; ku < w - w / 2; ++ku) {
+  for (int ku = -len / 2; ku < len - len / 2; ++ku) {
     cd s = 0;
-    for (int j = -w / 2; j < w - w / 2; ++j) {
-      double a = -2.0 * PI * (double)(((long long)ku * j) % w) / w;
+    for (int j = -len / 2; j < len - len / 2; ++j) {
+      double a = -2.0 * PI * (double)(((long long)ku * j) % len) / len;
       s += ramp_kernel(g.filter, j) * cd(cos(a), sin(a));
     }
-    Hk[ku + w / 2] = scale * s.real();
+    Hk[ku + len / 2] = scale * s.real();
+    if (g.filter == 3) Hk[ku + len / 2] *= parzen((double)ku / (0.5 * len));
   }
 }
+
+static void make_filter(const orc_geom& g, double* Hk) { make_filter_len(g, g.w, Hk); }
 
 extern "C" void orc_filter(const orc_geom* g, double* Hk) { make_filter(*g, Hk); }
 
@@ -180,9 +195,49 @@ extern "C" void orc_filter(const orc_geom* g, double* Hk) { make_filter(*g, Hk);
 //   u = j_u - c_u, v = j_v - c_v.
 // Rows then columns with the 1-D DFT above; the centring is the phase e^{+2 pi i k c / n}.
 // ---------------------------------------------------------------------------------------------
-static void spectrum(const orc_geom& g, const double* d, const double* Hk, cd* HD) {
+// Reading Q11b (u-padding, PAPER.md is silent): with g.pad > 1 every detector row is extended to pad*w samples by
+// replicating its two edge values ((pad-1) w / 2 samples on each side), filtered as a row of that length (the filter
+// response of the longer row, so that the convolution with the ramp kernel no longer wraps around the detector) and
+// cropped back to its w samples.  q[j_v][j_u], filter included.
+static void filter_rows_padded(const orc_geom& g, const double* d, double* q) {
+  int h = g.h, w = g.w, wp = g.pad * w, off = (wp - w) / 2;
+  std::vector<double> Hp(wp);
+  make_filter_len(g, wp, Hp.data());
+#pragma omp parallel for schedule(static)
+  for (int jv = 0; jv < h; ++jv) {
+    std::vector<cd> row(wp);
+    for (int j = 0; j < wp; ++j) {
+      int ju = j - off;
+      ju = ju < 0 ? 0 : (ju >= w ? w - 1 : ju);
+      row[j] = d[(size_t)jv * w + ju];
+    }
+    dft1(row.data(), wp, -1);
+    for (int k = -wp / 2; k < wp - wp / 2; ++k) row[(k + wp) % wp] *= Hp[k + wp / 2];
+    dft1(row.data(), wp, +1);
+    for (int ju = 0; ju < w; ++ju) q[(size_t)jv * w + ju] = row[ju + off].real() / wp;
+  }
+}
+
+extern "C" void orc_filter_rows_padded(const orc_geom* g, const void* proj, int th, double* q) {
+  std::vector<double> d((size_t)g->h * g->w);
+  load_proj(*g, proj, th, d.data());
+  filter_rows_padded(*g, d.data(), q);
+}
+
+static void spectrum(const orc_geom& g, const double* d_in, const double* Hk_in, cd* HD) {
   int h = g.h, w = g.w;
   std::vector<cd> tmp((size_t)h * w);
+  // padded rows: the filter has been applied in the space domain already, the transform below runs with H = 1
+  std::vector<double> qpad, ones;
+  const double* d = d_in;
+  const double* Hk = Hk_in;
+  if (g.pad > 1 && g.filter != 0) {
+    qpad.resize((size_t)h * w);
+    filter_rows_padded(g, d_in, qpad.data());
+    ones.assign(w, 1.0);
+    d = qpad.data();
+    Hk = ones.data();
+  }
 #pragma omp parallel for schedule(static)
   for (int jv = 0; jv < h; ++jv) {
     std::vector<cd> row(w);
@@ -202,6 +257,15 @@ static void spectrum(const orc_geom& g, const double* d, const double* Hk, cd* H
       double a = 2.0 * PI * kv * g.cv / h;
       HD[(size_t)(kv + h / 2) * w + iu] = col[(kv + h) % h] * cd(cos(a), sin(a)) / ((double)w * h);
     }
+  }
+  // 2-D spectral multiplier on the projection (PAPER.md:199, 279 name Paganin filtering as a pre-processing step; the
+  // single-distance Paganin filter is the low-pass 1/(1 + alpha |k|^2); reading Q17: applied to the line integrals)
+  if (g.alpha != 0.0) {
+    for (int kv = -h / 2; kv < h - h / 2; ++kv)
+      for (int ku = -w / 2; ku < w - w / 2; ++ku) {
+        double fu = (double)ku / w, fv = (double)kv / h;
+        HD[(size_t)(kv + h / 2) * w + (ku + w / 2)] /= 1.0 + g.alpha * (fu * fu + fv * fv);
+      }
   }
 }
 

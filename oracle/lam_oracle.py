@@ -29,7 +29,7 @@ class _Geom(C.Structure):
                 ("cu", C.c_double), ("cv", C.c_double),
                 ("filter", C.c_int), ("dtype", C.c_int),
                 ("dark", C.POINTER(C.c_float)), ("flat", C.POINTER(C.c_float)),
-                ("tmin", C.c_double)]
+                ("tmin", C.c_double), ("pad", C.c_int), ("alpha", C.c_double)]
 
 
 _lib = None
@@ -49,7 +49,7 @@ def lib():
     return _lib
 
 
-FILTERS = {"none": 0, "ramp": 1, "shepp-logan": 2}
+FILTERS = {"none": 0, "ramp": 1, "shepp-logan": 2, "parzen": 3}
 KERNELS = {"kb": 0, "gauss": 1}
 
 
@@ -57,7 +57,7 @@ class Geometry:
     """Scan geometry (Eq. 2 / Eq. 6) + filter choice + input encoding."""
 
     def __init__(self, n, h, w, theta, phi, nz=None, filter="ramp", cu=None, cv=None,
-                 dark=None, flat=None, tmin=1e-6):
+                 dark=None, flat=None, tmin=1e-6, pad=1, alpha=0.0):
         self.n, self.h, self.w = int(n), int(h), int(w)
         self.nz = int(nz) if nz else int(n)
         self.theta = np.ascontiguousarray(theta, dtype=np.float64)
@@ -69,6 +69,8 @@ class Geometry:
         self.dark = None if dark is None else np.ascontiguousarray(dark, dtype=np.float32)
         self.flat = None if flat is None else np.ascontiguousarray(flat, dtype=np.float32)
         self.tmin = float(tmin)
+        self.pad = int(pad)        # rows edge-extended to pad*w before the filter (reading Q11b)
+        self.alpha = float(alpha)  # 2-D spectral multiplier 1/(1 + alpha |k|^2) (reading Q17)
 
     def _c(self, proj):
         g = _Geom()
@@ -78,6 +80,7 @@ class Geometry:
         g.cu, g.cv = self.cu, self.cv
         g.filter = FILTERS[self.filter]
         g.tmin = self.tmin
+        g.pad, g.alpha = self.pad, self.alpha
         if proj is None:
             g.dtype = 0
         else:
@@ -118,6 +121,15 @@ def prep(geom, proj, th):
     out = np.empty((geom.h, geom.w))
     g = geom._c(proj)
     lib().orc_prep(C.byref(g), _p(proj), C.c_int(th), _p(out))
+    return out
+
+
+def filter_rows_padded(geom, proj, th):
+    """Rows of projection th filtered after edge extension to pad*w samples (reading Q11b) -> float64 [h][w]."""
+    assert geom.pad > 1
+    out = np.empty((geom.h, geom.w))
+    g = geom._c(proj)
+    lib().orc_filter_rows_padded(C.byref(g), _p(proj), C.c_int(th), _p(out))
     return out
 
 

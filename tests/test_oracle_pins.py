@@ -409,3 +409,80 @@ def test_paper_table1_gain_column_is_consistent():
     import os
     t = np.loadtxt(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_table1.txt"))
     assert np.all(np.abs(t[:, 4] / t[:, 3] - t[:, 5]) < 0.06)
+
+
+# ---- f4: Parzen window, u-padding, 2-D spectral multiplier -----------------------------------------
+def test_P12_parzen_window_is_the_fourfold_box_convolution():
+    """PAPER.md:109 names the Parzen low-pass.  The Parzen window is, independently of its piecewise-cubic formula,
+    the four-fold self-convolution of a box (cubic B-spline) normalised to 1 at the origin: checked on a fine grid,
+    plus the exact values P(0) = 1, P(1/2) = 1/4, P(1) = 0."""
+    w = 64
+    g_r = O.Geometry(32, 16, w, np.linspace(0, 2 * np.pi, 8, endpoint=False), 0.3, filter="ramp")
+    g_p = O.Geometry(32, 16, w, np.linspace(0, 2 * np.pi, 8, endpoint=False), 0.3, filter="parzen")
+    Hr, Hp = O.filter_response(g_r), O.filter_response(g_p)
+    k = np.arange(-w // 2, w // 2)
+    ratio = Hp[k != 0] / Hr[k != 0]
+    m = 4000                                   # samples per box; box width 1/2 so that the 4-fold convolution spans [-1, 1]
+    box = np.ones(m)
+    b4 = np.convolve(np.convolve(box, box), np.convolve(box, box)).astype(np.float64)
+    b4 /= b4.max()
+    xs = (np.arange(len(b4)) - (len(b4) - 1) / 2) / (2.0 * m)   # total support 4 m samples = 2 units
+    ref = np.interp(np.abs(k[k != 0]) / (w / 2), xs, b4)
+    assert np.abs(ratio - ref).max() < 2e-3
+    assert abs(Hp[w // 2 + w // 4] / Hr[w // 2 + w // 4] - 0.25) < 1e-12   # x = 1/2
+    assert abs(Hp[0]) < 1e-15                                              # x = 1 (Nyquist)
+    assert abs(Hp[w // 2 + 1] / Hr[w // 2 + 1] - (1 - 6 * (2 / w) ** 2 + 6 * (2 / w) ** 3)) < 1e-12
+
+
+def test_P13_padded_rows_are_a_linear_convolution_with_the_ramp_kernel():
+    """Reading Q11b: after edge extension to 2w samples the filter is the LINEAR convolution of the extended row with
+    the band-limited ramp kernel h_RL (h[0] = 1/4, h[odd j] = -1/(pi j)^2), truncated to |j| <= w: numpy.convolve of
+    the closed-form kernel samples is the library routine it must reduce to."""
+    rng = np.random.default_rng(5)
+    n, h, w, nth, phi = 16, 8, 32, 6, 0.35
+    theta = np.linspace(0, 2 * np.pi, nth, endpoint=False)
+    proj = rng.normal(size=(nth, h, w))
+    g = O.Geometry(n, h, w, theta, phi, filter="ramp", pad=2)
+    q = O.filter_rows_padded(g, proj, 2)
+    wp, off = 2 * w, w // 2
+    j = np.arange(-wp // 2, wp // 2)
+    hk = np.where(j == 0, 0.25, np.where(j % 2 == 0, 0.0, -1.0 / (np.pi * np.maximum(np.abs(j), 1)) ** 2))
+    scale = np.pi * np.cos(phi) / nth
+    for jv in (0, 3, 7):
+        ext = np.concatenate([np.full(off, proj[2, jv, 0]), proj[2, jv], np.full(off, proj[2, jv, -1])])
+        # circular convolution of length 2w == linear convolution wrapped once; written as the full linear
+        # convolution folded back modulo 2w (kernel index j = -w .. w-1)
+        lin = np.convolve(ext, hk)                       # index i <-> position i + j[0]
+        circ = np.zeros(wp)
+        for i, v in enumerate(lin):
+            circ[(i + j[0]) % wp] += v
+        assert np.abs(q[jv] - scale * circ[off:off + w]).max() < 1e-12
+    # and the point of padding: a constant row is filtered to (nearly) zero instead of wrapping edge to edge
+    gc = O.Geometry(n, h, w, theta, phi, filter="ramp", pad=2)
+    ramp = np.tile(np.linspace(0.0, 1.0, w), (nth, h, 1))
+    qp = O.filter_rows_padded(gc, ramp, 0)
+    g1 = O.Geometry(n, h, w, theta, phi, filter="ramp")
+    q1 = np.fft.ifft(np.fft.fft(ramp[0, 0]) * np.fft.ifftshift(O.filter_response(g1))).real
+    assert np.abs(qp[0]).max() < 0.25 * np.abs(q1).max()   # the unpadded filter sees the 1 -> 0 jump at the wrap
+
+
+def test_P14_spectral_multiplier_scales_a_plane_wave_exactly():
+    """Reading Q17: the 2-D multiplier 1/(1 + alpha ((k_u/w)^2 + (k_v/h)^2)).  A projection that is one plane wave
+    cos(2 pi (a u/w + b v/h)) has the two spectral bins (b, a) and (-b, -a) only; each must come out as
+    H[a] / 2 / (1 + alpha (a^2/w^2 + b^2/h^2)), and alpha = 0 must change nothing."""
+    n, h, w, nth, phi = 16, 16, 32, 4, 0.3
+    theta = np.linspace(0, 2 * np.pi, nth, endpoint=False)
+    a, b, alpha = 5, -3, 37.0
+    ju, jv = np.meshgrid(np.arange(w) - w / 2, np.arange(h) - h / 2)
+    proj = np.tile(np.cos(2 * np.pi * (a * ju / w + b * jv / h)), (nth, 1, 1))
+    g0 = O.Geometry(n, h, w, theta, phi, filter="ramp")
+    g1 = O.Geometry(n, h, w, theta, phi, filter="ramp", alpha=alpha)
+    H = O.filter_response(g0)
+    s0, s1 = O.spectrum(g0, proj, 1), O.spectrum(g1, proj, 1)
+    mult = 1.0 / (1.0 + alpha * ((a / w) ** 2 + (b / h) ** 2))
+    assert abs(s0[b + h // 2, a + w // 2] - 0.5 * H[a + w // 2]) < 1e-13
+    assert abs(s1[b + h // 2, a + w // 2] - 0.5 * H[a + w // 2] * mult) < 1e-13
+    assert abs(s1[-b + h // 2, -a + w // 2] - 0.5 * H[-a + w // 2] * mult) < 1e-13
+    mask = np.ones((h, w), bool)
+    mask[b + h // 2, a + w // 2] = mask[-b + h // 2, -a + w // 2] = False
+    assert np.abs(s1[mask]).max() < 1e-13
