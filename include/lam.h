@@ -13,7 +13,8 @@
  *     In formulas:  vol[x] = Re sum_theta sum_{k_v,k_u} H[k_u] D[theta,k_v,k_u] e^{+2 pi i x.xi},
  *         D = (1/(w h)) sum_{j_v,j_u} d[theta,j_v,j_u] e^{-2 pi i (k_u u/w + k_v v/h)},  u = j_u-c_u, v = j_v-c_v,
  *         H = (pi cos(phi)/N_theta) DFT_w(band-limited ramp kernel)   (reading Q3 of "a suitable scaled version
- *         of |sigma| cos(phi)"), Shepp-Logan variant, or H = 1 (pure adjoint L*).
+ *         of |sigma| cos(phi)"), its Shepp-Logan or Parzen-windowed low-pass variants,
+ *         or H = 1 (pure adjoint L*).
  *   lam_forward:      proj = L_phi vol = F*_2D F_u3D vol                   Eq. 5; the exact transpose
  *                     of lam_backproject with filter = LAM_FILTER_NONE (adjoint test <L f, d> = <f, L* d>).
  *   raw 16-bit input: d = -log( max( (raw-dark)/max(flat-dark,1), t_min ) ), the inverse of the detector model
@@ -65,7 +66,7 @@ typedef enum {
 } lam_status;
 
 enum { LAM_KERNEL_KB = 0, LAM_KERNEL_GAUSS = 1 };
-enum { LAM_FILTER_NONE = 0, LAM_FILTER_RAMP = 1, LAM_FILTER_SHEPP_LOGAN = 2 };
+enum { LAM_FILTER_NONE = 0, LAM_FILTER_RAMP = 1, LAM_FILTER_SHEPP_LOGAN = 2, LAM_FILTER_PARZEN = 3 };
 enum { LAM_INPUT_F32 = 0, LAM_INPUT_U16_RAW = 1 };
 
 typedef struct {
@@ -82,6 +83,12 @@ typedef struct {
   size_t device_bytes; /* workspace budget; 0 -> 90 % of the free device memory at lam_create               */
   int plane_batch;     /* k_v planes gridded + transformed per launch; 0 -> as many as fit 4 GB of fine grid  */
   int theta_chunk;     /* projections per filter/FFT launch (and per host->device copy); 0 -> auto          */
+  int pad_u;           /* 1: every detector row is extended to 2w samples by replicating its edge values before the
+                          filter and cropped after it, so that the ramp convolution does not wrap around the detector
+                          (reading Q11b; w <= 4096); 0: none (the circular filter of the definition)              */
+  float spectral_alpha;/* alpha >= 0 of the 2-D low-pass 1/(1 + alpha ((k_u/w)^2 + (k_v/h)^2)) applied to every
+                          projection spectrum: the single-distance Paganin multiplier named as pre-processing in
+                          PAPER.md:199, 279, applied to the line integrals (reading Q17); 0: none                 */
 } lam_params;
 
 /* Fill *p with the defaults (KB, W = 6, sigma = 2, ramp filter, fp32 input, centred axis). */
@@ -102,6 +109,19 @@ lam_status lam_set_darkflat(lam_plan* plan, const float* dark, const float* flat
 /* vol <- W L* proj (overwrites vol).  proj: float32 or uint16 per params.input.  See the header comment for
  * pointer kinds and stream semantics. */
 lam_status lam_backproject(lam_plan* plan, const void* proj, float* vol, void* cuda_stream);
+
+/* One x3-slice of lam_backproject for a list of rotation-axis positions: the `try` search of PAPER.md:254-270 ("run
+ * reconstruction of 1 slice for different rotation axes"); with plans created for different phi it is the
+ * `try-lamino` search.  out[c][i2][i1] (device, n_centers x n x n float32; n_centers = 0: one slice
+ * at the plan's own axis, centers_u may be NULL) is slice i3 (0 <= i3 < nz) of the volume lam_backproject would return
+ * with params.center_u = centers_u[c] (HOST array, pixels).  Evaluated as Eq. 9 with the x3
+ * transform done exactly: every k_v plane is gridded in (xi1, xi2), multiplied by e^{2 pi i x3 k_v cos(phi)/h} and
+ * added onto one fine grid, then one 2-D inverse FFT, crop and division by the kernel transform in x1, x2 (no x3
+ * gridding, so the slice differs from the full volume's by the x3 gridding error only, ~1e-5).  The axis position
+ * is a phase on the k_u spectra (reading Q13), re-applied per centre.  Device pointers only; asynchronous on
+ * cuda_stream except for two small table uploads; cost per centre ~ one S2 stage. */
+lam_status lam_backproject_slice(lam_plan* plan, const void* proj, int i3, int n_centers, const float* centers_u,
+                                 float* out, void* cuda_stream);
 
 /* proj <- L vol (overwrites proj, float32): Eq. 5 as the exact transpose, stage by stage in reverse
  * order, of lam_backproject with filter none (the plan's filter setting is ignored; an input plan of type uint16

@@ -12,6 +12,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -49,6 +50,7 @@ struct lam_plan {
   int M = 0, M3 = 0, W = 0, NP = 0, WR = 0, WQ = 0;
   int logw = 0, logh = 0, logM = 0, logM3 = 0;
   int PB = 1, TC = 1;  // plane batch, theta chunk
+  int TSB = 1;         // planes per x1/x2 sub-batch: T (the x1-transformed planes) is sized to stay L2-resident
   int rows_nb = 1, cols_lcb = 3, x1_nb = 1, x2_lnb = 3, KZ = 1, z_lcb = 3;
   GridKernel gk;
   KerPoly kp{};
@@ -56,6 +58,11 @@ struct lam_plan {
   // device tables
   double2* d_cs = nullptr;
   float2 *d_Pu = nullptr, *d_Pv = nullptr, *d_PuNone = nullptr;
+  float* d_Hp = nullptr;       // pad_u: filter response of the 2w-sample rows, k = 0..w, times 1/(2w)
+  float2* d_tw_w2 = nullptr;   // pad_u: twiddles of length 2w
+  int rows_nb_pad = 1;
+  // single-slice mode (allocated on first use): summed fine grid, its x1 transform, cropped plane, phase tables
+  float2 *d_Gs = nullptr, *d_Ts = nullptr, *d_As = nullptr, *d_zph = nullptr, *d_cph = nullptr;
   float2 *d_tw_w = nullptr, *d_tw_h = nullptr, *d_tw_M = nullptr, *d_tw_M3 = nullptr;
   float *d_ztab = nullptr, *d_zlast = nullptr, *d_dx = nullptr, *d_dz = nullptr, *d_dark = nullptr, *d_flat = nullptr;
   float2* d_df = nullptr;
@@ -63,6 +70,11 @@ struct lam_plan {
   int* d_bz = nullptr;    // [NP] first x3 tap per plane
   int *d_zlo = nullptr, *d_zcnt = nullptr, *d_zidx = nullptr;
   int nact = 0;  // active x3 grid cells
+  // x3 stage through TMA (k_zstage_tma): tensor map over A[p][x2][x1], box split, double-buffer size, launch shape
+  CUtensorMap tmapA;
+  bool z_tma = false;
+  int z_nbox = 1, z_pbox = 1, z_bufelems = 0, z_threads = 512, z_blocks_per_sm = 1, n_sm = 148;
+  size_t z_smem = 0;
   Job* d_jobs = nullptr;
   std::vector<long long> job_off;  // [batches+1] first job of each plane batch (jobs of a batch: heaviest tiles first)
   unsigned* d_multi = nullptr;     // tiles written by several jobs, batch-major
@@ -81,6 +93,18 @@ struct lam_plan {
   cudaEvent_t ev_in_ready[2] = {}, ev_in_free[2] = {}, ev_out_ready[2] = {}, ev_out_free[2] = {}, ev_fork = nullptr;
   bool host_path_ready = false;
   bool last_call_host = false;   // the last lam_backproject streamed through host pointers
+  // spilled (out-of-core) mode, chosen by lam_create when the in-core workspace exceeds params.device_bytes
+  // (PAPER.md:172 "> 64 GB for 2048^3", :181-191): the spectra S exist for one BAND of planes at a time (S0+S1 run once
+  // per band), the cropped planes A[p] leave for pinned host memory as their batch is born and come back per x2-slab
+  // for the x3 stage
+  bool spill = false;
+  int chunk_ctr = 0;                   // projection chunks issued by the current call (host-pointer path)
+  int band = 0;                        // planes per band (a multiple of PB)
+  int ZRs = 0;                         // x2 rows per x3-stage slab
+  float2* h_A = nullptr;               // pinned host [NP][n][n]
+  float2* d_Ab[2] = {nullptr, nullptr};  // device staging of one plane batch of A
+  float2* d_As2[2] = {nullptr, nullptr}; // device slab [NP][ZRs][n]
+  cudaEvent_t ev_ab_ready[2] = {}, ev_ab_free[2] = {}, ev_sl_ready[2] = {}, ev_sl_free[2] = {};
   // bookkeeping
   std::string err;
   int device = 0;
@@ -167,6 +191,18 @@ struct Launch {
       note_launch();
     }
   }
+  static void rows_pad(bool raw, dim3 g, size_t sm, cudaStream_t s, const RowsPadArgs& a) {
+    if constexpr (L < kLogMax) {
+      if (raw) {
+        cudaFuncSetAttribute(k_rows_pad<L, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        k_rows_pad<L, true><<<g, 256, sm, s>>>(a);
+      } else {
+        cudaFuncSetAttribute(k_rows_pad<L, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+        k_rows_pad<L, false><<<g, 256, sm, s>>>(a);
+      }
+      note_launch();
+    }
+  }
   static void cols(dim3 g, int threads, size_t sm, cudaStream_t s, const ColsArgs& a) {
     cudaFuncSetAttribute(k_cols<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
     k_cols<L><<<g, threads, sm, s>>>(a);
@@ -207,9 +243,20 @@ struct Launch {
     k_rows_T<L><<<g, 256, sm, s>>>(a);
     note_launch();
   }
-  static void z(dim3 g, size_t sm, cudaStream_t s, const ZArgs& a) {
+  static void ztma(int grid, int threads, size_t sm, cudaStream_t s, const CUtensorMap& tm, const ZTmaArgs& a) {
+    cudaFuncSetAttribute(k_zstage_tma<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    k_zstage_tma<L><<<grid, threads, sm, s>>>(tm, a);
+    note_launch();
+  }
+  static int ztma_occupancy(int threads, size_t sm) {
+    cudaFuncSetAttribute(k_zstage_tma<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_zstage_tma<L>, threads, sm) != cudaSuccess) { cudaGetLastError(); nb = 0; }
+    return nb;
+  }
+  static void z(dim3 g, int threads, size_t sm, cudaStream_t s, const ZArgs& a) {
     cudaFuncSetAttribute(k_zstage<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    k_zstage<L><<<g, 512, sm, s>>>(a);
+    k_zstage<L><<<g, threads, sm, s>>>(a);
       note_launch();
   }
 };
@@ -254,7 +301,7 @@ struct StageScope {
 
 void free_all(lam_plan* p) {
   void* ptrs[] = {p->d_cs,    p->d_Pu,  p->d_Pv,  p->d_PuNone, p->d_tw_w, p->d_tw_h,   p->d_tw_M, p->d_tw_M3,
-                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_zcnt, p->d_zidx, p->d_df, p->d_wz, p->d_bz, p->d_multi,
+                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_Hp, p->d_tw_w2, p->d_Gs, p->d_Ts, p->d_As, p->d_zph, p->d_cph, p->d_zcnt, p->d_zidx, p->d_df, p->d_wz, p->d_bz, p->d_multi,
                   p->d_R,     p->d_arena, p->d_G, p->d_T};
   for (void* q : ptrs)
     if (q) cudaFree(q);
@@ -266,6 +313,15 @@ void free_all(lam_plan* p) {
     if (p->ev_out_ready[i]) cudaEventDestroy(p->ev_out_ready[i]);
     if (p->ev_out_free[i]) cudaEventDestroy(p->ev_out_free[i]);
   }
+  for (int i = 0; i < 2; ++i) {
+    if (p->d_Ab[i]) cudaFree(p->d_Ab[i]);
+    if (p->d_As2[i]) cudaFree(p->d_As2[i]);
+    if (p->ev_ab_ready[i]) cudaEventDestroy(p->ev_ab_ready[i]);
+    if (p->ev_ab_free[i]) cudaEventDestroy(p->ev_ab_free[i]);
+    if (p->ev_sl_ready[i]) cudaEventDestroy(p->ev_sl_ready[i]);
+    if (p->ev_sl_free[i]) cudaEventDestroy(p->ev_sl_free[i]);
+  }
+  if (p->h_A) cudaFreeHost(p->h_A);
   if (p->ev_fork) cudaEventDestroy(p->ev_fork);
   if (p->s_h2d) cudaStreamDestroy(p->s_h2d);
   if (p->s_d2h) cudaStreamDestroy(p->s_d2h);
@@ -382,6 +438,14 @@ lam_status make_tables(lam_plan* p) {
     Pv[q] = make_float2((float)std::cos(a), (float)std::sin(a));
   }
   if ((st = upload(p, &p->d_Pv, Pv)) != LAM_OK) return st;
+  if (p->prm.pad_u) {
+    std::vector<double> H2;
+    filter_response(p->prm.filter, 2 * w, p->phi, p->ntheta, H2);  // k = 0..w
+    std::vector<float> Hp(w + 1);
+    for (int k = 0; k <= w; ++k) Hp[k] = (float)(H2[k] / (2.0 * w));
+    if ((st = upload(p, &p->d_Hp, Hp)) != LAM_OK) return st;
+    if ((st = upload(p, &p->d_tw_w2, twiddles(2 * w))) != LAM_OK) return st;
+  }
   if ((st = upload(p, &p->d_tw_w, twiddles(w))) != LAM_OK) return st;
   if ((st = upload(p, &p->d_tw_h, twiddles(h))) != LAM_OK) return st;
   if ((st = upload(p, &p->d_tw_M, twiddles(M))) != LAM_OK) return st;
@@ -464,8 +528,87 @@ lam_status make_tables(lam_plan* p) {
 }
 
 size_t zstage_smem(const lam_plan* p, int cb) {
-  const size_t work = std::max((size_t)p->NP * z_pitch(cb), (size_t)cb * fft_tfast_pitch(p->M3, cb));
+  const size_t work = std::max((size_t)p->NP * z_pitch(cb), (size_t)(cb / 2) * fft_tfast_pitch(p->M3, cb / 2));
   return (((work + 1) & ~(size_t)1) + (size_t)p->nact * cb) * sizeof(float2);
+}
+
+// x3 stage through TMA: tensor map of A viewed as [p][x2][x1] of 8-byte elements, boxes of pbox planes x cb columns
+size_t ztma_smem(const lam_plan* p, int cb, int* nbox, int* pbox, int* bufelems) {
+  const int nb = (p->NP + 255) / 256;
+  int pb = (p->NP + nb - 1) / nb;
+  pb = (pb + 7) & ~7;  // every box lands 128-byte aligned for cb >= 2
+  if (pb > 256) pb = 256;
+  const size_t ain = (size_t)nb * pb * cb, fft = (size_t)(cb / 2) * fft_tfast_pitch(p->M3, cb / 2);
+  const size_t be = (std::max(ain, fft) + 15) & ~(size_t)15;
+  *nbox = nb; *pbox = pb; *bufelems = (int)be;
+  return (2 * be + (size_t)p->nact * cb) * sizeof(float2) + 16;
+}
+
+void setup_ztma(lam_plan* p) {
+  p->z_tma = false;
+  {
+    int nsm = 0;
+    if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, p->device) == cudaSuccess && nsm > 0) p->n_sm = nsm;
+    else cudaGetLastError();
+  }
+  {  // block size of the plain kernel: fewest idle lanes over the rounds of its gridding phase (nact * cb/2 tasks)
+    const int total = p->nact * ((1 << p->z_lcb) / 2);
+    long bestcost = -1;
+    for (int T = 384; T <= 512; T += 32) {
+      const long cost = (long)((total + T - 1) / T) * T;
+      if (bestcost < 0 || cost < bestcost || (cost == bestcost && T > p->z_threads)) { bestcost = cost; p->z_threads = T; }
+    }
+    if (const char* e = getenv("LAM_TUNE_ZTHREADS")) p->z_threads = std::min(512, atoi(e));
+  }
+  // The TMA-pipelined persistent form (k_zstage_tma) is kept for reference: measured SLOWER than the plain kernel
+  // (configs[2] 4.06 against 3.68 ms, configs[3] 60 against 44 ms), so it is opt-in.
+  const char* ez = getenv("LAM_TUNE_ZTMA");
+  if (!ez || atoi(ez) == 0 || p->spill) return;
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    return;
+  }
+  // columns per block: the largest of 8, 4, 2 whose double buffer lets two blocks share an SM, else the largest that fits
+  int lcb = 3, lmax = 3;
+  if (const char* e = getenv("LAM_TUNE_ZLCB")) lcb = lmax = std::max(1, std::min(4, atoi(e)));
+  int nbox, pbox, be;
+  while (lcb > 1 && ztma_smem(p, 1 << lcb, &nbox, &pbox, &be) > 112 * 1024) --lcb;
+  if (ztma_smem(p, 1 << lcb, &nbox, &pbox, &be) > 112 * 1024) {
+    lcb = lmax;
+    while (lcb > 1 && ztma_smem(p, 1 << lcb, &nbox, &pbox, &be) > 226 * 1024) --lcb;
+  }
+  const size_t sm = ztma_smem(p, 1 << lcb, &nbox, &pbox, &be);
+  if (sm > 226 * 1024 || (p->n % (1 << lcb)) != 0) return;
+  const int cb = 1 << lcb;
+  cuuint64_t gdim[3] = {(cuuint64_t)p->n, (cuuint64_t)p->n, (cuuint64_t)p->NP};
+  cuuint64_t gstr[2] = {(cuuint64_t)p->n * 8, (cuuint64_t)p->n * p->n * 8};
+  cuuint32_t box[3] = {(cuuint32_t)cb, 1, (cuuint32_t)pbox};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = ((encode_fn)fn)(&p->tmapA, CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, (void*)p->d_A, gdim, gstr, box, estr,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return;
+  // block size: fewest wasted lanes over the rounds of phase 2 (nact * 8 tasks), 384..640 threads
+  const int total = p->nact * 8;
+  int best = 512;
+  long bestcost = -1;
+  for (int T = 384; T <= 640; T += 32) {
+    const long cost = (long)((total + T - 1) / T) * T;
+    if (bestcost < 0 || cost < bestcost || (cost == bestcost && T > best)) { bestcost = cost; best = T; }
+  }
+  if (const char* e = getenv("LAM_TUNE_ZTHREADS")) best = atoi(e);
+  int occ = 0;
+  dispatch_log_impl<kLogMin>(p->logM3, [&](auto L_) { occ = decltype(L_)::ztma_occupancy(best, sm); });
+  if (occ < 1) return;
+  p->z_lcb = lcb; p->z_nbox = nbox; p->z_pbox = pbox; p->z_bufelems = be; p->z_threads = best; p->z_blocks_per_sm = occ;
+  p->z_smem = sm;
+  p->z_tma = true;
 }
 
 }  // namespace
@@ -491,6 +634,8 @@ void lam_default_params(lam_params* p) {
   p->device_bytes = 0;
   p->plane_batch = 0;
   p->theta_chunk = 0;
+  p->pad_u = 0;
+  p->spectral_alpha = 0.f;
 }
 
 const char* lam_last_error(const lam_plan* plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
@@ -518,7 +663,10 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   if ((n | h | w | P.nz) & 1) return fail(nullptr, LAM_EINVAL, "n, nz, h, w must be even");
   if (!(phi_rad >= 0.f) || !(phi_rad < 1.5707963f)) return fail(nullptr, LAM_EINVAL, "phi must be in [0, pi/2)");
   if (P.kernel != LAM_KERNEL_KB && P.kernel != LAM_KERNEL_GAUSS) return fail(nullptr, LAM_EINVAL, "unknown kernel");
-  if (P.filter < 0 || P.filter > 2) return fail(nullptr, LAM_EINVAL, "unknown filter");
+  if (P.filter < 0 || P.filter > 3) return fail(nullptr, LAM_EINVAL, "unknown filter");
+  if (!(P.spectral_alpha >= 0.f)) return fail(nullptr, LAM_EINVAL, "spectral_alpha must be >= 0");
+  if (P.pad_u != 0 && P.pad_u != 1) return fail(nullptr, LAM_EINVAL, "pad_u must be 0 or 1");
+  if (P.pad_u && w > 4096) return fail(nullptr, LAM_EUNSUPPORTED, "pad_u needs w <= 4096 (rows of 2w samples)");
   if (P.input != LAM_INPUT_F32 && P.input != LAM_INPUT_U16_RAW) return fail(nullptr, LAM_EINVAL, "unknown input type");
   if (P.width != 4 && P.width != 6 && P.width != 8) return fail(nullptr, LAM_EUNSUPPORTED, "width must be 4, 6 or 8");
   if (!(P.oversample >= 1.25f) || !(P.oversample <= 4.f)) return fail(nullptr, LAM_EINVAL, "oversample must be in [1.25, 4]");
@@ -560,6 +708,7 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
 
   // block shapes
   p->rows_nb = std::min(h / 2, std::max(1, 4096 / w));
+  p->rows_nb_pad = std::min(h / 2, std::max(1, 1024 / w));  // two buffers of 2w samples per row pair
   p->x1_nb = std::max(1, std::min(M, 4096 / M));
   auto tfast_lognb = [](int len, int lmax = 3) { int l = lmax; while (l > 0 && (size_t)(1 << l) * fft_tfast_pitch(len, 1 << l) * 8 > 200 * 1024) --l; return l; };
   p->cols_lcb = tfast_lognb(h);
@@ -583,15 +732,63 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   // share one arena: A grows from the front, S sits right-aligned at the back; a batch of PB planes may be in flight.
   const size_t splane = (size_t)n_theta * p->WQ, aplane = (size_t)n * n;
   const size_t arena = std::max((size_t)p->PB * aplane + (size_t)p->NP * splane, (size_t)p->NP * aplane + (size_t)p->PB * splane);
-  const size_t need = (size_t)p->TC * rproj + arena * 8 + (size_t)p->PB * (gplane + tplane) + p->device_bytes;
-  if (need > budget)
-    return bail(fail(p, LAM_ENOMEM_DEVICE, "in-core workspace of %.2f GB exceeds the budget of %.2f GB", need / 1e9, budget / 1e9));
-  if ((st = dalloc(p, &p->d_R, (size_t)p->TC * h * p->WR)) != LAM_OK) return bail(st);
-  if ((st = dalloc(p, &p->d_arena, arena)) != LAM_OK) return bail(st);
-  p->d_A = p->d_arena;
-  p->d_S = p->d_arena + (arena - (size_t)p->NP * splane);
+  // T holds the x1-transformed planes of one sub-batch.  Measured (configs[2], [3]): sub-batches small enough to keep T
+  // in L2 (1-4 planes) are SLOWER than whole batches (S3 13.7 / 11.6 / 11.1 ms at 1 / 2 / 4 planes against 9.7 ms): the
+  // passes are issue-bound, not HBM-bound, and short launches pay their tails.  So T covers the whole plane batch.
+  p->TSB = p->PB;
+  if (const char* e = getenv("LAM_TUNE_TSB")) p->TSB = std::max(1, std::min(p->PB, atoi(e)));
+  // the gridding work lists are allocated by build_jobs: about one 32-byte job per (plane, tile)
+  const size_t jobs_est = (size_t)((double)p->NP * (M / kTS) * (M / kTS) * 1.1) * sizeof(Job);
+  const size_t need = (size_t)p->TC * rproj + arena * 8 + (size_t)p->PB * gplane + (size_t)p->TSB * tplane + jobs_est + p->device_bytes;
+  if (need <= budget && !getenv("LAM_TUNE_FORCE_SPILL")) {
+    if ((st = dalloc(p, &p->d_R, (size_t)p->TC * h * p->WR)) != LAM_OK) return bail(st);
+    if ((st = dalloc(p, &p->d_arena, arena)) != LAM_OK) return bail(st);
+    p->d_A = p->d_arena;
+    p->d_S = p->d_arena + (arena - (size_t)p->NP * splane);
+  } else {
+    // ---- spilled mode: size every buffer from the budget ----
+    p->spill = true;
+    const size_t left0 = budget > jobs_est + p->device_bytes ? budget - jobs_est - p->device_bytes : 0;
+    if (P.theta_chunk <= 0) p->TC = (int)std::max<size_t>(1, std::min<size_t>(p->TC, left0 / 16 / rproj));
+    const size_t per_plane = gplane + tplane + 2 * aplane * 8;  // G, T and the two staging copies of the cropped plane
+    if (P.plane_batch <= 0) p->PB = (int)std::max<size_t>(1, std::min<size_t>(p->PB, left0 / 4 / per_plane));
+    p->TSB = p->PB;
+    const size_t slab_row = (size_t)p->NP * n * 8;               // one x2 row of every plane
+    p->ZRs = (int)std::max<size_t>(1, std::min<size_t>(n, left0 / 8 / (2 * slab_row)));
+    while (n % p->ZRs) --p->ZRs;
+    const size_t fixed = (size_t)p->TC * rproj + (size_t)p->PB * per_plane + 2 * (size_t)p->ZRs * slab_row;
+    const size_t sbytes = splane * 8;
+    size_t nband = left0 > fixed ? (left0 - fixed) / sbytes : 0;
+    nband = std::min<size_t>(nband, p->NP);
+    nband -= nband % p->PB;
+    if (nband < (size_t)p->PB)
+      return bail(fail(p, LAM_ENOMEM_DEVICE, "budget of %.2f GB is too small even for the spilled schedule (needs %.2f GB for one batch of %d planes)",
+                       budget / 1e9, (fixed + (size_t)p->PB * sbytes + jobs_est + p->device_bytes) / 1e9, p->PB));
+    p->band = (int)nband;
+    if ((st = dalloc(p, &p->d_R, (size_t)p->TC * h * p->WR)) != LAM_OK) return bail(st);
+    if ((st = dalloc(p, &p->d_arena, (size_t)p->band * splane)) != LAM_OK) return bail(st);
+    p->d_S = p->d_arena;
+    p->d_A = nullptr;
+    for (int i = 0; i < 2; ++i) {
+      if ((st = dalloc(p, &p->d_Ab[i], (size_t)p->PB * aplane)) != LAM_OK) return bail(st);
+      if ((st = dalloc(p, &p->d_As2[i], (size_t)p->NP * p->ZRs * n)) != LAM_OK) return bail(st);
+      cudaEventCreateWithFlags(&p->ev_ab_ready[i], cudaEventDisableTiming);
+      cudaEventCreateWithFlags(&p->ev_ab_free[i], cudaEventDisableTiming);
+      cudaEventCreateWithFlags(&p->ev_sl_ready[i], cudaEventDisableTiming);
+      cudaEventCreateWithFlags(&p->ev_sl_free[i], cudaEventDisableTiming);
+    }
+    const size_t hbytes = (size_t)p->NP * aplane * 8;
+    if (cudaHostAlloc((void**)&p->h_A, hbytes, cudaHostAllocDefault) != cudaSuccess) {
+      cudaGetLastError();
+      p->h_A = nullptr;
+      return bail(fail(p, LAM_ENOMEM_HOST, "spilled schedule: %.2f GB of pinned host memory for the cropped planes could not be allocated", hbytes / 1e9));
+    }
+    p->pinned_bytes += hbytes;
+    p->ZR = p->ZRs;  // output slabs of the host-pointer path follow the x3-stage slabs
+  }
   if ((st = dalloc(p, &p->d_G, (size_t)p->PB * M * M)) != LAM_OK) return bail(st);
-  if ((st = dalloc(p, &p->d_T, (size_t)p->PB * M * n)) != LAM_OK) return bail(st);
+  if ((st = dalloc(p, &p->d_T, (size_t)p->TSB * M * n)) != LAM_OK) return bail(st);
+  setup_ztma(p);
   if ((st = build_jobs(p)) != LAM_OK) return bail(st);
   if (cudaDeviceSynchronize() != cudaSuccess) return bail(fail(p, LAM_ECUDA, "plan setup failed: %s", cudaGetErrorString(cudaGetLastError())));
   *out = p;
@@ -632,26 +829,38 @@ static bool is_device_ptr(const void* q) {
 }
 
 // S0 + S1 for projections [th0, th0 + nth) at device pointer `chunk` (the first projection of the chunk)
-static void launch_s1(lam_plan* p, const void* chunk, int th0, int nth, cudaStream_t s) {
+static void launch_s1(lam_plan* p, const void* chunk, int th0, int nth, cudaStream_t s, int p_lo = 0, int p_hi = 1 << 30) {
   if (p->copy_only) return;
   const bool raw = p->prm.input == LAM_INPUT_U16_RAW;
-  RowsArgs ra{chunk, p->d_df, p->prm.t_min, p->d_R, p->d_Pu, p->d_tw_w, p->h, p->WR, p->rows_nb};
-  dim3 gr(p->h / 2 / p->rows_nb, nth);
-  size_t smr = (size_t)p->rows_nb * fft_span(p->w) * sizeof(float2);
-  DISPATCH_LOG(p->logw, rows(raw, gr, smr, s, ra));
+  if (p->prm.pad_u && p->prm.filter != LAM_FILTER_NONE) {
+    RowsPadArgs pa{{chunk, p->d_df, p->prm.t_min, p->d_R, p->d_PuNone, p->d_tw_w, p->h, p->WR, p->rows_nb_pad}, p->d_Hp, p->d_tw_w2};
+    dim3 gr(p->h / 2 / p->rows_nb_pad, nth);
+    size_t smr = (size_t)2 * p->rows_nb_pad * fft_span(2 * p->w) * sizeof(float2);
+    DISPATCH_LOG(p->logw, rows_pad(raw, gr, smr, s, pa));
+  } else {
+    RowsArgs ra{chunk, p->d_df, p->prm.t_min, p->d_R, p->d_Pu, p->d_tw_w, p->h, p->WR, p->rows_nb};
+    dim3 gr(p->h / 2 / p->rows_nb, nth);
+    size_t smr = (size_t)p->rows_nb * fft_span(p->w) * sizeof(float2);
+    DISPATCH_LOG(p->logw, rows(raw, gr, smr, s, ra));
+  }
   const int cb = 1 << p->cols_lcb;
-  ColsArgs ca{p->d_R, p->d_S, p->d_Pv, p->d_tw_h, p->w, p->WR, p->WQ, p->ntheta, th0, p->cols_lcb};
+  // banded (spilled) mode: the stored band starts at plane p_lo; the kernels index planes absolutely
+  float2* S0 = p->d_S - (size_t)(p->spill ? p_lo : 0) * p->ntheta * p->WQ;
+  ColsArgs ca{p->d_R, S0, p->d_Pv, p->d_tw_h, p->w, p->WR, p->WQ, p->ntheta, th0, p->cols_lcb, p_lo, p_hi, p->prm.spectral_alpha};
   dim3 gc((p->w / 2 + 1 + cb - 1) / cb, nth);
   size_t smc = (size_t)cb * fft_tfast_pitch(p->h, cb) * sizeof(float2);
   DISPATCH_LOG(p->logh, cols(gc, (size_t)cb * p->h >= 16384 ? 512 : 256, smc, s, ca));
   p->launches += 2;
 }
 
-// S2 + S3 (x1, x2) for planes [p0, p0 + np): p0 is a multiple of the plane batch
-static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
+// S2 + S3 (x1, x2) for planes [p0, p0 + np): p0 is a multiple of the plane batch.  slice = true: S2 only, then the
+// planes are added, each times its x3 phase, onto the single fine grid of lam_backproject_slice.
+static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s, bool slice = false, float2* Aout = nullptr, int band_lo = 0) {
   if (p->copy_only) return;
+  if (!Aout) Aout = p->d_A + (size_t)p0 * p->n * p->n;
   const int b = p0 / p->PB;
-  SpreadArgs sa{p->geom, p->kp, p->d_jobs + p->job_off[b], p->job_off[b + 1] - p->job_off[b], p->d_S, p->WQ, p->d_G, p0,
+  SpreadArgs sa{p->geom, p->kp, p->d_jobs + p->job_off[b], p->job_off[b + 1] - p->job_off[b],
+                p->d_S - (size_t)band_lo * p->ntheta * p->WQ, p->WQ, p->d_G, p0,
                 p->d_multi + p->multi_off[b], p->multi_off[b + 1] - p->multi_off[b]};
   {
     StageScope sc(p, 1, s);
@@ -668,33 +877,68 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s) {
       note_launch();
     });
   }
-  {
-    StageScope sc(p, 2, s);
-    IfftArgs a1{p->d_G, p->d_T, p->d_tw_M, p->n, p->x1_nb, 0};
-    DISPATCH_LOG(p->logM, x1(dim3(p->M / p->x1_nb, np), (size_t)p->x1_nb * fft_span(p->M) * sizeof(float2), s, a1));
-    const int nb2 = 1 << p->x2_lnb;
-    IfftArgs a2{p->d_T, p->d_A + (size_t)p0 * p->n * p->n, p->d_tw_M, p->n, nb2, p->x2_lnb};
-    DISPATCH_LOG(p->logM, x2(dim3(p->n / nb2, np), (size_t)nb2 * p->M >= 16384 ? 512 : 256,
-                             (size_t)nb2 * fft_tfast_pitch(p->M, nb2) * sizeof(float2), s, a2));
+  if (slice) {
+    const size_t cells = (size_t)p->M * p->M;
+    k_slice_reduce<<<p->n_sm * 8, 256, 0, s>>>(p->d_G, p->d_Gs, p->d_zph + p0, np, cells);
+    note_launch();
+    p->launches += 2;
+    return;
   }
-  p->launches += 3;
+  {
+    // x1 then x2 on sub-batches of TSB planes through ONE small T buffer: T is written and re-read while it is still
+    // in L2 (its lines are overwritten by the next sub-batch before they are evicted), so only G and A move through HBM
+    StageScope sc(p, 2, s);
+    const int nb2 = 1 << p->x2_lnb;
+    for (int q = 0; q < np; q += p->TSB) {
+      const int nq = std::min(p->TSB, np - q);
+      IfftArgs a1{p->d_G + (size_t)q * p->M * p->M, p->d_T, p->d_tw_M, p->n, p->x1_nb, 0};
+      DISPATCH_LOG(p->logM, x1(dim3(p->M / p->x1_nb, nq), (size_t)p->x1_nb * fft_span(p->M) * sizeof(float2), s, a1));
+      IfftArgs a2{p->d_T, Aout + (size_t)q * p->n * p->n, p->d_tw_M, p->n, nb2, p->x2_lnb};
+      DISPATCH_LOG(p->logM, x2(dim3(p->n / nb2, nq), (size_t)nb2 * p->M >= 16384 ? 512 : 256,
+                               (size_t)nb2 * fft_tfast_pitch(p->M, nb2) * sizeof(float2), s, a2));
+      p->launches += 2;
+    }
+  }
+  p->launches += 1;
 }
 
 // x3 stage for x2 rows [x2_0, x2_0 + rows); out holds x2 row `out_x2_0` in its first row, z-stride `zstride` floats
-static void launch_z(lam_plan* p, float* out, size_t zstride, int x2_0, int rows, int out_x2_0, cudaStream_t s) {
+static void launch_z(lam_plan* p, float* out, size_t zstride, int x2_0, int rows, int out_x2_0, cudaStream_t s,
+                     const float2* Abuf = nullptr, size_t a_pstride = 0, int a_x2_0 = 0) {
   if (p->copy_only) return;
   StageScope sc(p, 3, s);
-  ZArgs za{p->d_A, out, zstride, p->d_tw_M3, p->d_ztab, p->d_zlo, p->d_zcnt, p->d_zlast, p->d_zidx, p->d_dx, p->d_dz,
+  if (!Abuf) { Abuf = p->d_A; a_pstride = (size_t)p->n * p->n; a_x2_0 = 0; }
+  ZArgs za{Abuf, a_pstride, a_x2_0, out, zstride, p->d_tw_M3, p->d_ztab, p->d_zlo, p->d_zcnt, p->d_zlast, p->d_zidx, p->d_dx, p->d_dz,
            p->n, p->nz, p->NP, p->nact, p->z_lcb, x2_0, out_x2_0};
-  DISPATCH_LOG(p->logM3, z(dim3(p->n >> p->z_lcb, rows), zstage_smem(p, 1 << p->z_lcb), s, za));
+  if (p->z_tma) {
+    ZTmaArgs ta{za, p->n >> p->z_lcb, rows * (p->n >> p->z_lcb), p->z_nbox, p->z_pbox, p->z_bufelems};
+    const int grid = std::min(ta.nitems, p->n_sm * p->z_blocks_per_sm);
+    DISPATCH_LOG(p->logM3, ztma(grid, p->z_threads, p->z_smem, s, p->tmapA, ta));
+  } else {
+    DISPATCH_LOG(p->logM3, z(dim3(p->n >> p->z_lcb, rows), p->z_threads, zstage_smem(p, 1 << p->z_lcb), s, za));
+  }
   p->launches += 1;
+}
+
+static lam_status init_copy_streams(lam_plan* p) {
+  if (p->s_h2d) return LAM_OK;
+  CU(p, cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming));
+  CU(p, cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
+  CU(p, cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
+  return LAM_OK;
 }
 
 static lam_status init_host_path(lam_plan* p) {
   if (p->host_path_ready) return LAM_OK;
+  {
+    lam_status st0 = init_copy_streams(p);
+    if (st0 != LAM_OK) return st0;
+  }
   const size_t esz = p->prm.input == LAM_INPUT_U16_RAW ? 2 : 4;
-  p->ZR = (int)std::max<size_t>(1, std::min<size_t>(p->n, ((size_t)256 << 20) / ((size_t)p->nz * p->n * 4)));
-  while (p->n % p->ZR) --p->ZR;
+  if (p->ZR == 0) {
+    p->ZR = (int)std::max<size_t>(1, std::min<size_t>(p->n, ((size_t)256 << 20) / ((size_t)p->nz * p->n * 4)));
+    while (p->n % p->ZR) --p->ZR;
+  }
   lam_status st;
   for (int i = 0; i < 2; ++i) {
     char* q = nullptr;
@@ -706,10 +950,44 @@ static lam_status init_host_path(lam_plan* p) {
     CU(p, cudaEventCreateWithFlags(&p->ev_out_ready[i], cudaEventDisableTiming));
     CU(p, cudaEventCreateWithFlags(&p->ev_out_free[i], cudaEventDisableTiming));
   }
-  CU(p, cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming));
-  CU(p, cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking));
-  CU(p, cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking));
   p->host_path_ready = true;
+  return LAM_OK;
+}
+
+// S0 + S1 over every projection for the planes [p_lo, p_hi) (all planes in core; one band in spilled mode).  Device
+// projections are read in place; host projections stream in chunks on the copy stream, double-buffered against the
+// kernels.  p->chunk_ctr numbers the chunks of the whole call: the two staging buffers alternate
+// across bands as well.
+static lam_status run_s1_all(lam_plan* p, const void* proj, bool proj_dev, cudaStream_t s, int p_lo, int p_hi) {
+  const size_t esz = p->prm.input == LAM_INPUT_U16_RAW ? 2 : 4;
+  const size_t pbytes = (size_t)p->h * p->w * esz;
+  if (proj_dev) {
+    StageScope sc(p, 0, s);
+    for (int th0 = 0; th0 < p->ntheta; th0 += p->TC) {
+      int nth = std::min(p->TC, p->ntheta - th0);
+      launch_s1(p, (const char*)proj + (size_t)th0 * pbytes, th0, nth, s, p_lo, p_hi);
+    }
+    return LAM_OK;
+  }
+  if (p->chunk_ctr == 0) {
+    CU(p, cudaEventRecord(p->ev_fork, s));
+    CU(p, cudaStreamWaitEvent(p->s_h2d, p->ev_fork, 0));
+  }
+  for (int th0 = 0; th0 < p->ntheta; th0 += p->TC, ++p->chunk_ctr) {
+    const int nth = std::min(p->TC, p->ntheta - th0), c = p->chunk_ctr, b = c & 1;
+    if (c >= 2) CU(p, cudaStreamWaitEvent(p->s_h2d, p->ev_in_free[b], 0));
+    {
+      StageScope sc(p, 4, p->s_h2d);
+      CU(p, cudaMemcpyAsync(p->d_in[b], (const char*)proj + (size_t)th0 * pbytes, (size_t)nth * pbytes, cudaMemcpyHostToDevice, p->s_h2d));
+    }
+    CU(p, cudaEventRecord(p->ev_in_ready[b], p->s_h2d));
+    CU(p, cudaStreamWaitEvent(s, p->ev_in_ready[b], 0));
+    {
+      StageScope sc(p, 0, s);
+      launch_s1(p, p->d_in[b], th0, nth, s, p_lo, p_hi);
+    }
+    CU(p, cudaEventRecord(p->ev_in_free[b], s));
+  }
   return LAM_OK;
 }
 
@@ -724,43 +1002,81 @@ lam_status lam_backproject(lam_plan* p, const void* proj, float* vol, void* cuda
     lam_status st = init_host_path(p);
     if (st != LAM_OK) return st;
   }
+  if (p->spill) {
+    lam_status st = init_copy_streams(p);
+    if (st != LAM_OK) return st;
+  }
   p->launches = 0;
   g_launch_error = cudaSuccess;
   p->events_used = 0;
   p->stage_valid = false;
-  const size_t esz = p->prm.input == LAM_INPUT_U16_RAW ? 2 : 4;
-  const size_t pbytes = (size_t)p->h * p->w * esz;
   {
     StageScope total(p, 5, s);
-    if (proj_dev) {
-      StageScope sc(p, 0, s);
-      for (int th0 = 0; th0 < p->ntheta; th0 += p->TC) {
-        int nth = std::min(p->TC, p->ntheta - th0);
-        launch_s1(p, (const char*)proj + (size_t)th0 * pbytes, th0, nth, s);
+    {
+      p->chunk_ctr = 0;
+      lam_status st0 = run_s1_all(p, proj, proj_dev, s, 0, p->spill ? p->band : (1 << 30));
+      if (st0 != LAM_OK) return st0;
+    }
+    if (!p->spill)
+      for (int p0 = 0; p0 < p->NP; p0 += p->PB) launch_planes(p, p0, std::min(p->PB, p->NP - p0), s);
+    if (p->spill) {
+      // ---- spilled schedule: bands of planes; band 0 has been transformed above, the others repeat S0+S1 ----
+      const size_t aplane = (size_t)p->n * p->n;
+      int nb_done = 0;
+      for (int p_lo = 0; p_lo < p->NP; p_lo += p->band) {
+        const int p_hi = std::min(p->NP, p_lo + p->band);
+        if (p_lo > 0) {
+          lam_status st1 = run_s1_all(p, proj, proj_dev, s, p_lo, p_hi);
+          if (st1 != LAM_OK) return st1;
+        }
+        for (int p0 = p_lo; p0 < p_hi; p0 += p->PB, ++nb_done) {
+          const int np = std::min(p->PB, p_hi - p0), b = nb_done & 1;
+          if (nb_done >= 2) CU(p, cudaStreamWaitEvent(s, p->ev_ab_free[b], 0));
+          launch_planes(p, p0, np, s, false, p->d_Ab[b], p_lo);
+          CU(p, cudaEventRecord(p->ev_ab_ready[b], s));
+          CU(p, cudaStreamWaitEvent(p->s_d2h, p->ev_ab_ready[b], 0));
+          {
+            StageScope sc(p, 4, p->s_d2h);
+            CU(p, cudaMemcpyAsync(p->h_A + (size_t)p0 * aplane, p->d_Ab[b], (size_t)np * aplane * sizeof(float2), cudaMemcpyDeviceToHost, p->s_d2h));
+          }
+          CU(p, cudaEventRecord(p->ev_ab_free[b], p->s_d2h));
+        }
       }
-    } else {
-      // projections stream host -> device in chunks on the copy stream, double-buffered against S0+S1
-      CU(p, cudaEventRecord(p->ev_fork, s));
-      CU(p, cudaStreamWaitEvent(p->s_h2d, p->ev_fork, 0));
+      CU(p, cudaEventRecord(p->ev_fork, p->s_d2h));
+      CU(p, cudaStreamWaitEvent(p->s_h2d, p->ev_fork, 0));  // the slabs are read back only after the last plane has left
+      CU(p, cudaStreamWaitEvent(s, p->ev_fork, 0));
       int c = 0;
-      for (int th0 = 0; th0 < p->ntheta; th0 += p->TC, ++c) {
-        int nth = std::min(p->TC, p->ntheta - th0), b = c & 1;
-        if (c >= 2) CU(p, cudaStreamWaitEvent(p->s_h2d, p->ev_in_free[b], 0));
+      for (int r0 = 0; r0 < p->n; r0 += p->ZRs, ++c) {
+        const int b = c & 1;
+        if (c >= 2) CU(p, cudaStreamWaitEvent(p->s_h2d, p->ev_sl_free[b], 0));
         {
           StageScope sc(p, 4, p->s_h2d);
-          CU(p, cudaMemcpyAsync(p->d_in[b], (const char*)proj + (size_t)th0 * pbytes, (size_t)nth * pbytes, cudaMemcpyHostToDevice, p->s_h2d));
+          CU(p, cudaMemcpy2DAsync(p->d_As2[b], (size_t)p->ZRs * p->n * sizeof(float2), p->h_A + (size_t)r0 * p->n, aplane * sizeof(float2),
+                                  (size_t)p->ZRs * p->n * sizeof(float2), p->NP, cudaMemcpyHostToDevice, p->s_h2d));
         }
-        CU(p, cudaEventRecord(p->ev_in_ready[b], p->s_h2d));
-        CU(p, cudaStreamWaitEvent(s, p->ev_in_ready[b], 0));
-        {
-          StageScope sc(p, 0, s);
-          launch_s1(p, p->d_in[b], th0, nth, s);
+        CU(p, cudaEventRecord(p->ev_sl_ready[b], p->s_h2d));
+        CU(p, cudaStreamWaitEvent(s, p->ev_sl_ready[b], 0));
+        if (vol_dev) {
+          launch_z(p, vol, (size_t)p->n * p->n, r0, p->ZRs, 0, s, p->d_As2[b], (size_t)p->ZRs * p->n, r0);
+        } else {
+          if (c >= 2) CU(p, cudaStreamWaitEvent(s, p->ev_out_free[b], 0));
+          launch_z(p, p->d_out[b], (size_t)p->ZR * p->n, r0, p->ZRs, r0, s, p->d_As2[b], (size_t)p->ZRs * p->n, r0);
+          CU(p, cudaEventRecord(p->ev_out_ready[b], s));
+          CU(p, cudaStreamWaitEvent(p->s_d2h, p->ev_out_ready[b], 0));
+          {
+            StageScope sc(p, 4, p->s_d2h);
+            CU(p, cudaMemcpy2DAsync(vol + (size_t)r0 * p->n, (size_t)p->n * p->n * 4, p->d_out[b], (size_t)p->ZR * p->n * 4,
+                                    (size_t)p->ZR * p->n * 4, p->nz, cudaMemcpyDeviceToHost, p->s_d2h));
+          }
+          CU(p, cudaEventRecord(p->ev_out_free[b], p->s_d2h));
         }
-        CU(p, cudaEventRecord(p->ev_in_free[b], s));
+        CU(p, cudaEventRecord(p->ev_sl_free[b], s));
       }
-    }
-    for (int p0 = 0; p0 < p->NP; p0 += p->PB) launch_planes(p, p0, std::min(p->PB, p->NP - p0), s);
-    if (vol_dev) {
+      if (!vol_dev) {
+        CU(p, cudaEventRecord(p->ev_fork, p->s_d2h));
+        CU(p, cudaStreamWaitEvent(s, p->ev_fork, 0));
+      }
+    } else if (vol_dev) {
       launch_z(p, vol, (size_t)p->n * p->n, 0, p->n, 0, s);
     } else {
       // volume leaves in slabs of ZR x2-rows, double-buffered against the x3 stage
@@ -786,8 +1102,83 @@ lam_status lam_backproject(lam_plan* p, const void* proj, float* vol, void* cuda
   if (g_launch_error != cudaSuccess) return fail(p, LAM_ECUDA, "kernel launch failed: %s", cudaGetErrorString(g_launch_error));
   p->stage_valid = p->profiling;
   p->last_call_host = !proj_dev || !vol_dev;
+  if (p->spill) CU(p, cudaStreamSynchronize(p->s_d2h));  // the pinned plane store is plan-owned: nothing of it is in flight on return
   if (!proj_dev) CU(p, cudaStreamSynchronize(p->s_h2d));  // the caller's host projections are consumed on return
   if (!vol_dev) CU(p, cudaStreamSynchronize(p->s_d2h));   // host results are valid on return
+  return LAM_OK;
+}
+
+lam_status lam_backproject_slice(lam_plan* p, const void* proj, int i3, int n_centers, const float* centers_u, float* out,
+                                 void* cuda_stream) {
+  if (!p) return LAM_EINVAL;
+  if (!proj || !out) return fail(p, LAM_EINVAL, "proj / out is NULL");
+  if (i3 < 0 || i3 >= p->nz) return fail(p, LAM_EINVAL, "slice index %d outside [0, %d)", i3, p->nz);
+  if (n_centers < 0 || (n_centers > 0 && !centers_u)) return fail(p, LAM_EINVAL, "n_centers < 0 or centers_u is NULL");
+  if (p->prm.input == LAM_INPUT_U16_RAW && !p->have_darkflat) return fail(p, LAM_EINVAL, "uint16 input needs lam_set_darkflat first");
+  cudaSetDevice(p->device);
+  if (!is_device_ptr(proj) || !is_device_ptr(out)) return fail(p, LAM_EUNSUPPORTED, "lam_backproject_slice takes device pointers only");
+  if (p->spill) return fail(p, LAM_EUNSUPPORTED, "lam_backproject_slice needs the in-core workspace (the plan runs the spilled schedule)");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const int n = p->n, M = p->M, NP = p->NP, w = p->w, h = p->h;
+  lam_status st;
+  if (!p->d_Gs) {
+    if ((st = dalloc(p, &p->d_Gs, (size_t)M * M)) != LAM_OK) return st;
+    if ((st = dalloc(p, &p->d_Ts, (size_t)M * n)) != LAM_OK) return st;
+    if ((st = dalloc(p, &p->d_As, (size_t)n * n)) != LAM_OK) return st;
+    if ((st = dalloc(p, &p->d_zph, (size_t)NP)) != LAM_OK) return st;
+    if ((st = dalloc(p, &p->d_cph, (size_t)p->WQ)) != LAM_OK) return st;
+  }
+  p->launches = 0;
+  g_launch_error = cudaSuccess;
+  p->stage_valid = false;
+  // exact x3 phase of every plane: e^{2 pi i x3 k_v cos(phi) / h}, x3 = i3 - nz/2 (Eq. 9)
+  {
+    std::vector<float2> zph(NP);
+    const double x3 = (double)(i3 - p->nz / 2), cphi = std::cos(p->phi);
+    for (int q = 0; q < NP; ++q) {
+      const int kv = q == h / 2 ? -h / 2 : q;
+      const double a = 2.0 * kPi * std::fmod(x3 * kv * cphi / h, 1.0);
+      zph[q] = make_float2((float)std::cos(a), (float)std::sin(a));
+    }
+    CU(p, cudaMemcpyAsync(p->d_zph, zph.data(), NP * sizeof(float2), cudaMemcpyHostToDevice, s));
+    CU(p, cudaStreamSynchronize(s));  // the pageable source vector dies with this scope
+  }
+  const size_t esz = p->prm.input == LAM_INPUT_U16_RAW ? 2 : 4;
+  const size_t pbytes = (size_t)h * w * esz;
+  for (int th0 = 0; th0 < p->ntheta; th0 += p->TC)
+    launch_s1(p, (const char*)proj + (size_t)th0 * pbytes, th0, std::min(p->TC, p->ntheta - th0), s);
+  const double cu0 = std::isnan(p->prm.center_u) ? 0.5 * w : (double)p->prm.center_u;
+  double cu_now = cu0;
+  const int nc = std::max(1, n_centers);
+  std::vector<float2> cph(p->WQ);
+  for (int ic = 0; ic < nc; ++ic) {
+    const double cu = n_centers > 0 ? (double)centers_u[ic] : cu0, delta = cu - cu_now;
+    if (delta != 0.0) {  // move the rotation axis by delta pixels: a phase on k_u (reading Q13), applied to S in place
+      for (int q = 0; q <= w; ++q) {
+        const double a = 2.0 * kPi * std::fmod((double)(q - w / 2) * delta / w, 1.0);
+        cph[q] = make_float2((float)std::cos(a), (float)std::sin(a));
+      }
+      CU(p, cudaMemcpyAsync(p->d_cph, cph.data(), (size_t)(w + 1) * sizeof(float2), cudaMemcpyHostToDevice, s));
+      CU(p, cudaStreamSynchronize(s));
+      k_center_shift<<<dim3((w + 1 + 127) / 128, 1024), 128, 0, s>>>(p->d_S, p->d_cph, p->WQ, w + 1, (size_t)NP * p->ntheta);
+      note_launch();
+      p->launches += 1;
+      cu_now = cu;
+    }
+    CU(p, cudaMemsetAsync(p->d_Gs, 0, (size_t)M * M * sizeof(float2), s));
+    for (int p0 = 0; p0 < NP; p0 += p->PB) launch_planes(p, p0, std::min(p->PB, NP - p0), s, true);
+    IfftArgs a1{p->d_Gs, p->d_Ts, p->d_tw_M, n, p->x1_nb, 0};
+    DISPATCH_LOG(p->logM, x1(dim3(M / p->x1_nb, 1), (size_t)p->x1_nb * fft_span(M) * sizeof(float2), s, a1));
+    const int nb2 = 1 << p->x2_lnb;
+    IfftArgs a2{p->d_Ts, p->d_As, p->d_tw_M, n, nb2, p->x2_lnb};
+    DISPATCH_LOG(p->logM, x2(dim3(n / nb2, 1), (size_t)nb2 * M >= 16384 ? 512 : 256,
+                             (size_t)nb2 * fft_tfast_pitch(M, nb2) * sizeof(float2), s, a2));
+    k_slice_out<<<(unsigned)(((size_t)n * n + 255) / 256), 256, 0, s>>>(p->d_As, out + (size_t)ic * n * n, p->d_dx, n);
+    note_launch();
+    p->launches += 3;
+  }
+  CU(p, cudaGetLastError());
+  if (g_launch_error != cudaSuccess) return fail(p, LAM_ECUDA, "kernel launch failed: %s", cudaGetErrorString(g_launch_error));
   return LAM_OK;
 }
 
@@ -796,6 +1187,7 @@ lam_status lam_forward(lam_plan* p, const float* vol, float* proj, void* cuda_st
   if (!vol || !proj) return fail(p, LAM_EINVAL, "vol / proj is NULL");
   cudaSetDevice(p->device);
   if (!is_device_ptr(vol) || !is_device_ptr(proj)) return fail(p, LAM_EUNSUPPORTED, "lam_forward takes device pointers only");
+  if (p->spill) return fail(p, LAM_EUNSUPPORTED, "lam_forward needs the in-core workspace (the plan runs the spilled schedule)");
   cudaStream_t s = (cudaStream_t)cuda_stream;
   p->launches = 0;
   g_launch_error = cudaSuccess;
@@ -812,18 +1204,22 @@ lam_status lam_forward(lam_plan* p, const float* vol, float* proj, void* cuda_st
   // planes, last batch first (the spectra planes are written right-aligned into the arena the A^T planes leave)
   for (int p0 = ((NP - 1) / p->PB) * p->PB; p0 >= 0; p0 -= p->PB) {
     const int np = std::min(p->PB, NP - p0), nb2 = 1 << p->x2_lnb;
-    IfftArgs a2{p->d_A + (size_t)p0 * n * n, p->d_T, p->d_tw_M, n, nb2, p->x2_lnb};
-    DISPATCH_LOG(p->logM, x2T(dim3(n / nb2, np), (size_t)nb2 * M >= 16384 ? 512 : 256,
-                              (size_t)nb2 * fft_tfast_pitch(M, nb2) * sizeof(float2), s, a2));
-    IfftArgs a1{p->d_T, p->d_G, p->d_tw_M, n, p->x1_nb, 0};
-    DISPATCH_LOG(p->logM, x1T(dim3(M / p->x1_nb, np), (size_t)p->x1_nb * fft_span(M) * sizeof(float2), s, a1));
+    for (int q = 0; q < np; q += p->TSB) {
+      const int nq = std::min(p->TSB, np - q);
+      IfftArgs a2{p->d_A + (size_t)(p0 + q) * n * n, p->d_T, p->d_tw_M, n, nb2, p->x2_lnb};
+      DISPATCH_LOG(p->logM, x2T(dim3(n / nb2, nq), (size_t)nb2 * M >= 16384 ? 512 : 256,
+                                (size_t)nb2 * fft_tfast_pitch(M, nb2) * sizeof(float2), s, a2));
+      IfftArgs a1{p->d_T, p->d_G + (size_t)q * M * M, p->d_tw_M, n, p->x1_nb, 0};
+      DISPATCH_LOG(p->logM, x1T(dim3(M / p->x1_nb, nq), (size_t)p->x1_nb * fft_span(M) * sizeof(float2), s, a1));
+      p->launches += 2;
+    }
     GatherArgs ga{p->geom, p->kp, p->d_G, p->d_S, p->WQ, p0, np};
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;
       k_gather<W><<<dim3((p->w + 1 + 255) / 256, p->ntheta, np), 256, 0, s>>>(ga);
       note_launch();
     });
-    p->launches += 3;
+    p->launches += 1;
   }
   // (S1)^T: un-fold + inverse FFT along v, then inverse FFT along u; H = 1 (the filter is not part of L)
   const int cb = 1 << p->cols_lcb, nbr = std::max(1, std::min(p->h, 4096 / p->w));
@@ -862,7 +1258,7 @@ lam_status lam_plan_info(const lam_plan* p, long long info[8]) {
   info[1] = p->NP;
   info[2] = p->PB;
   info[3] = p->job_off.empty() ? 0 : p->job_off.back();
-  info[4] = p->last_call_host ? 1 : 0;
+  info[4] = (p->last_call_host ? 1 : 0) | (p->spill ? 2 : 0);
   info[5] = p->TC;
   info[6] = p->launches;
   info[7] = (long long)p->pinned_bytes;

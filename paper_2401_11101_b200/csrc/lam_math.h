@@ -103,7 +103,7 @@ inline void kernel_poly(const GridKernel& gk, float* E /*[W/2][4]*/, float* O /*
 }
 
 inline double ramp_spatial(int filter, int j) {
-  if (filter == 1) {
+  if (filter == 1 || filter == 3) {
     if (j == 0) return 0.25;
     if (j & 1) return -1.0 / (kPi * kPi * (double)j * (double)j);
     return 0.0;
@@ -128,6 +128,10 @@ inline void filter_response(int filter, int w, double phi, int ntheta, std::vect
       s += hs[j + w / 2] * cs[m];
     }
     H[k] = scale * s;
+    if (filter == 3) {  // Parzen window over the ramp: x = k / (w/2), 1 at DC, 0 at Nyquist
+      const double x = (double)k / (0.5 * w);
+      H[k] *= x <= 0.5 ? 1.0 - 6.0 * x * x * (1.0 - x) : 2.0 * (1.0 - x) * (1.0 - x) * (1.0 - x);
+    }
   }
 }
 

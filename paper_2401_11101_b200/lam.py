@@ -19,7 +19,7 @@ INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LAM_OK, LAM_EINVAL, LAM_ENOMEM_DEVICE, LAM_ENOMEM_HOST, LAM_ECUDA, LAM_EUNSUPPORTED = range(6)
 STATUS_NAMES = ["LAM_OK", "LAM_EINVAL", "LAM_ENOMEM_DEVICE", "LAM_ENOMEM_HOST", "LAM_ECUDA", "LAM_EUNSUPPORTED"]
 KERNELS = {"kb": 0, "gauss": 1}
-FILTERS = {"none": 0, "ramp": 1, "shepp-logan": 2}
+FILTERS = {"none": 0, "ramp": 1, "shepp-logan": 2, "parzen": 3}
 INPUTS = {"f32": 0, "u16": 1}
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -30,7 +30,7 @@ class lam_params(C.Structure):
     _fields_ = [("nz", C.c_int), ("kernel", C.c_int), ("width", C.c_int), ("oversample", C.c_float),
                 ("shape", C.c_float), ("filter", C.c_int), ("input", C.c_int), ("center_u", C.c_float),
                 ("center_v", C.c_float), ("t_min", C.c_float), ("device_bytes", C.c_size_t),
-                ("plane_batch", C.c_int), ("theta_chunk", C.c_int)]
+                ("plane_batch", C.c_int), ("theta_chunk", C.c_int), ("pad_u", C.c_int), ("spectral_alpha", C.c_float)]
 
 
 class LamError(RuntimeError):
@@ -75,6 +75,7 @@ def lib():
     L.lam_set_darkflat.argtypes = [P, P, P]
     L.lam_backproject.argtypes = [P, P, P, P]
     L.lam_forward.argtypes = [P, P, P, P]
+    L.lam_backproject_slice.argtypes = [P, P, C.c_int, C.c_int, C.POINTER(C.c_float), P, P]
     L.lam_stage_ms.argtypes = [P, C.POINTER(C.c_float)]
     L.lam_set_profiling.argtypes = [P, C.c_int]
     L.lam_plan_info.argtypes = [P, C.POINTER(C.c_longlong)]
@@ -85,6 +86,7 @@ def lib():
 
 
 EXPORTS = ["lam_version", "lam_default_params", "lam_create", "lam_set_darkflat", "lam_backproject", "lam_forward",
+           "lam_backproject_slice",
            "lam_stage_ms", "lam_set_profiling", "lam_plan_info", "lam_last_error", "lam_destroy"]
 
 
@@ -126,6 +128,13 @@ def lam_backproject(plan, proj_ptr, vol_ptr, stream=0):
     _check(lib().lam_backproject(plan, C.c_void_p(proj_ptr), C.c_void_p(vol_ptr), C.c_void_p(stream)), plan)
 
 
+def lam_backproject_slice(plan, proj_ptr, i3, centers, out_ptr, stream=0):
+    """centers: sequence of rotation-axis positions (pixels, host) or None / empty for the plan's own axis."""
+    nc = len(centers) if centers is not None else 0
+    arr = (C.c_float * nc)(*[float(c) for c in centers]) if nc else None
+    _check(lib().lam_backproject_slice(plan, C.c_void_p(proj_ptr), int(i3), nc, arr, C.c_void_p(out_ptr), C.c_void_p(stream)), plan)
+
+
 def lam_forward(plan, vol_ptr, proj_ptr, stream=0):
     _check(lib().lam_forward(plan, C.c_void_p(vol_ptr), C.c_void_p(proj_ptr), C.c_void_p(stream)), plan)
 
@@ -154,7 +163,8 @@ def lam_destroy(plan):
 # ---- convenience wrapper over torch tensors --------------------------------------------------------------------------
 class Plan:
     def __init__(self, n, h, w, theta, phi, nz=None, kernel="kb", width=6, oversample=2.0, shape=0.0, filter="ramp",
-                 input="f32", center_u=None, center_v=None, t_min=1e-6, device_bytes=0, plane_batch=0, theta_chunk=0):
+                 input="f32", center_u=None, center_v=None, t_min=1e-6, device_bytes=0, plane_batch=0, theta_chunk=0,
+                 pad_u=False, spectral_alpha=0.0):
         p = lam_default_params()
         p.nz = int(nz or n)
         p.kernel, p.width, p.oversample, p.shape = KERNELS[kernel], int(width), float(oversample), float(shape)
@@ -163,6 +173,7 @@ class Plan:
         p.center_v = math.nan if center_v is None else float(center_v)
         p.t_min, p.device_bytes = float(t_min), int(device_bytes)
         p.plane_batch, p.theta_chunk = int(plane_batch), int(theta_chunk)
+        p.pad_u, p.spectral_alpha = int(bool(pad_u)), float(spectral_alpha)
         self.n, self.nz, self.h, self.w, self.ntheta = int(n), p.nz, int(h), int(w), len(theta)
         self.input = input
         self._plan = lam_create(n, h, w, theta, phi, p)
@@ -182,6 +193,19 @@ class Plan:
             stream = torch.cuda.current_stream().cuda_stream
         lam_backproject(self._plan, proj.data_ptr(), vol.data_ptr(), stream)
         return vol
+
+    def backproject_slice(self, proj, i3, centers=None, out=None, stream=None):
+        """Slice i3 for each rotation-axis position in `centers` (the `try` search) -> [nc][n][n]."""
+        import torch
+        assert proj.is_contiguous() and tuple(proj.shape) == (self.ntheta, self.h, self.w) and proj.is_cuda
+        nc = len(centers) if centers is not None and len(centers) else 1
+        if out is None:
+            out = torch.empty((nc, self.n, self.n), dtype=torch.float32, device=proj.device)
+        assert out.is_contiguous() and out.dtype == torch.float32 and tuple(out.shape) == (nc, self.n, self.n)
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        lam_backproject_slice(self._plan, proj.data_ptr(), i3, centers, out.data_ptr(), stream)
+        return out
 
     def forward(self, vol, proj=None, stream=None):
         import torch
