@@ -127,6 +127,42 @@ def test_config3_full_size_raw_uint16():
     print(f"configs[3] full size, data at {K} of {cfg.ntheta} random angles ({100.0 * K / cfg.ntheta:.1f} % of theta): {msg}; plan = {info}")
 
 
+def test_config3_full_size_spilled_with_a_16_GB_budget():
+    """S5 at full size: configs[3] needs 41 GB in core; with params.device_bytes = 16 GB the plan runs the spilled
+    schedule: spectra in bands of planes (S0+S1 once per band), the 34 GB of cropped planes
+    through plan-owned pinned host memory, the x3 stage per x2-slab.  Same checks as the in-core run."""
+    import psutil
+    cfg = inputs.config(3)
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60e9 or psutil.virtual_memory().available < 60e9:
+        pytest.skip("needs ~35 GB of device memory (scan + budget) and ~35 GB of pinned host memory")
+    rng = np.random.default_rng(SEED + 5)
+    K = 64
+    proj, sel, raw_sel, dark, flat = sparse_raw_scan(cfg, K, rng, "cuda")
+    try:
+        plan = lam.Plan(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
+                        input="u16", device_bytes=16 << 30)
+    except lam.LamError as e:
+        if e.status == lam.LAM_ENOMEM_HOST:
+            pytest.skip(f"cannot pin the host plane store: {e}")
+        raise
+    info = plan.info()
+    assert info["out_of_core"] & 2 and info["device_bytes"] <= 16 << 30 and info["pinned_bytes"] >= 34e9, info
+    plan.set_darkflat(dark.cuda(), flat.cuda())
+    vol = torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, device="cuda")
+    plan.backproject(proj, vol)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    plan.backproject(proj, vol)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    plan.close()
+    del proj
+    torch.cuda.empty_cache()
+    msg = check_raw(cfg, vol, sel, raw_sel, dark, flat, rng)
+    print(f"configs[3] spilled, 16 GB budget: {dt:.2f} s per call ({cfg.voxels / dt / 1e9:.2f} GVoxel/s), {msg}; plan = {info}")
+
+
 def test_config4_out_of_core_host_buffers():
     """configs[4]: 4096 x 4096 x 1024 volume (64 GiB) from 3000 uint16 projections of 2048 x 4096 (47 GiB), both in
     pinned HOST memory; lam_backproject streams chunks in and slabs out on its copy streams."""
