@@ -129,6 +129,22 @@ lam_status lam_backproject_slice(lam_plan* plan, const void* proj, int i3, int n
  * cuda_stream.  <L f, d> = <f, L* d> holds to fp32 rounding (about 1e-6 relative).  Not tuned. */
 lam_status lam_forward(lam_plan* plan, const float* vol, float* proj, void* cuda_stream);
 
+/* TV-regularised reconstruction of PAPER.md Appendix A (Eqs. 10-20):
+ *     minimise over mu   1/2 || L mu - d ||^2 + alpha || |grad mu| ||_1                                   (Eq. 10-11)
+ * by ADMM on the splitting grad mu = psi (Eqs. 12-16), starting from zeros: n_outer iterations of
+ *   (14) n_cg conjugate-gradient steps on F(mu) = 1/2 ||L mu - d||^2 + rho/2 ||grad mu - psi + lambda/rho||^2 (Eq. 17,
+ *        gradient Eq. 18) with Dai-Yuan directions (Eq. 19) and the exact step along each direction (F is quadratic),
+ *   (15) psi = shrink(grad mu + lambda/rho, alpha/rho), the isotropic soft threshold (Eq. 20 re-derived from Eq. 13:
+ *        the printed factors 2 do not satisfy the optimality condition; reading Q18),
+ *   (16) lambda += rho (grad mu - psi).
+ * L = lam_forward, L^T = lam_backproject of THIS plan, which must have been created with LAM_FILTER_NONE, fp32 input,
+ * no padding and no spectral multiplier (else LAM_EINVAL).  grad: forward differences, zero at the far faces.
+ * proj: the data d, [n_theta][h][w] float32; vol: the result mu (overwritten); both DEVICE pointers.
+ * history: NULL, or a HOST array of n_outer * n_cg doubles that receives ||grad F|| after every CG step.
+ * The call synchronises cuda_stream twice per CG step (the step lengths are host scalars). */
+lam_status lam_admm_tv(lam_plan* plan, const float* proj, float* vol, float alpha, float rho, int n_outer, int n_cg,
+                       double* history, void* cuda_stream);
+
 /* Per-stage device times of the LAST lam_backproject, milliseconds, measured with CUDA events on the plan's
  * streams when profiling is on (lam_set_profiling(plan, 1); it adds event records but no synchronisation inside
  * the call; this function synchronises).  ms[0] prep + filter + 2-D FFT (S0+S1), ms[1] gridding in (xi1,xi2)

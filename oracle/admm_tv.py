@@ -60,9 +60,10 @@ def lagrangian(Lmu_minus_d, gmu, psi, lam, alpha, rho):
             + float((lam * (gmu - psi)).sum()) + 0.5 * rho * float(((gmu - psi) ** 2).sum()))
 
 
-def admm_tv(geom, d, alpha, rho, n_outer, n_cg, L=None, LT=None):
+def admm_tv(geom, d, alpha, rho, n_outer, n_cg, L=None, LT=None, track=True):
     """geom: O.Geometry with filter "none".  d: projections [ntheta][h][w] (float64).
-    Returns mu and a history dict (F before/after every CG step, Lagrangian per outer iteration, psi, lam)."""
+    Returns mu and a history dict (||grad F|| after every CG step, psi, lam; with track: F before/after every CG step and
+    the Lagrangian per outer iteration, which cost one more application of L each)."""
     assert geom.filter == "none"
     if L is None:
         L = lambda f: O.forward_nudft(geom, f)
@@ -82,7 +83,8 @@ def admm_tv(geom, d, alpha, rho, n_outer, n_cg, L=None, LT=None):
     for k in range(n_outer):
         g = gradF(mu)
         eta = -g
-        hist["F"].append(F(mu))
+        if track:
+            hist["F"].append(F(mu))
         for m in range(n_cg):
             Leta, Geta = L(eta), grad(eta)
             gamma = -float((g * eta).sum()) / (float((Leta ** 2).sum()) + rho * float((Geta ** 2).sum()))  # reading Q19
@@ -91,11 +93,14 @@ def admm_tv(geom, d, alpha, rho, n_outer, n_cg, L=None, LT=None):
             beta = float((g_new ** 2).sum()) / float(((g_new - g) * eta).sum())                             # Eq. 19
             eta = -g_new + beta * eta
             g = g_new
-            hist["F"].append(F(mu))
+            hist.setdefault("gnorm_steps", []).append(float(np.sqrt((g ** 2).sum())))
+            if track:
+                hist["F"].append(F(mu))
         hist["gradF_norm"].append(float(np.sqrt((g ** 2).sum())))
         gmu = grad(mu)
         psi = shrink(gmu + lam / rho, alpha / rho)    # Eq. 15 / 20 (reading Q18)
         lam = lam + rho * (gmu - psi)                 # Eq. 16
-        hist["lagr"].append(lagrangian(L(mu) - d, gmu, psi, lam, alpha, rho))
+        if track:
+            hist["lagr"].append(lagrangian(L(mu) - d, gmu, psi, lam, alpha, rho))
     hist["psi"], hist["lam"] = psi, lam
     return mu, hist

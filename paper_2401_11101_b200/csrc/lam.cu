@@ -21,6 +21,7 @@
 #include "lam_kernels.cuh"
 #include "lam_spread.cuh"
 #include "lam_forward.cuh"
+#include "lam_admm.cuh"
 
 using namespace lam;
 
@@ -63,6 +64,10 @@ struct lam_plan {
   int rows_nb_pad = 1;
   // single-slice mode (allocated on first use): summed fine grid, its x1 transform, cropped plane, phase tables
   float2 *d_Gs = nullptr, *d_Ts = nullptr, *d_As = nullptr, *d_zph = nullptr, *d_cph = nullptr;
+  // ADMM-TV workspace (allocated on first use): gradient, direction, H eta (volumes), psi, lambda (3 volumes each), one
+  // projection-sized buffer, four double accumulators
+  float *d_tv_g = nullptr, *d_tv_eta = nullptr, *d_tv_h = nullptr, *d_tv_psi = nullptr, *d_tv_lam = nullptr, *d_tv_r = nullptr;
+  double* d_tv_acc = nullptr;
   float2 *d_tw_w = nullptr, *d_tw_h = nullptr, *d_tw_M = nullptr, *d_tw_M3 = nullptr;
   float *d_ztab = nullptr, *d_zlast = nullptr, *d_dx = nullptr, *d_dz = nullptr, *d_dark = nullptr, *d_flat = nullptr;
   float2* d_df = nullptr;
@@ -301,7 +306,7 @@ struct StageScope {
 
 void free_all(lam_plan* p) {
   void* ptrs[] = {p->d_cs,    p->d_Pu,  p->d_Pv,  p->d_PuNone, p->d_tw_w, p->d_tw_h,   p->d_tw_M, p->d_tw_M3,
-                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_Hp, p->d_tw_w2, p->d_Gs, p->d_Ts, p->d_As, p->d_zph, p->d_cph, p->d_zcnt, p->d_zidx, p->d_df, p->d_wz, p->d_bz, p->d_multi,
+                  p->d_ztab,  p->d_dx,  p->d_dz,  p->d_dark,   p->d_flat, p->d_zlo,    p->d_zlast,  p->d_jobs, p->d_Hp, p->d_tw_w2, p->d_Gs, p->d_Ts, p->d_As, p->d_zph, p->d_cph, p->d_tv_g, p->d_tv_eta, p->d_tv_h, p->d_tv_psi, p->d_tv_lam, p->d_tv_r, p->d_tv_acc, p->d_zcnt, p->d_zidx, p->d_df, p->d_wz, p->d_bz, p->d_multi,
                   p->d_R,     p->d_arena, p->d_G, p->d_T};
   for (void* q : ptrs)
     if (q) cudaFree(q);
@@ -1234,6 +1239,94 @@ lam_status lam_forward(lam_plan* p, const float* vol, float* proj, void* cuda_st
   }
   CU(p, cudaGetLastError());
   if (g_launch_error != cudaSuccess) return fail(p, LAM_ECUDA, "kernel launch failed: %s", cudaGetErrorString(g_launch_error));
+  return LAM_OK;
+}
+
+lam_status lam_admm_tv(lam_plan* p, const float* proj, float* vol, float alpha, float rho, int n_outer, int n_cg, double* history,
+                       void* cuda_stream) {
+  if (!p) return LAM_EINVAL;
+  if (!proj || !vol) return fail(p, LAM_EINVAL, "proj / vol is NULL");
+  if (!(alpha >= 0.f) || !(rho > 0.f) || n_outer < 1 || n_cg < 1) return fail(p, LAM_EINVAL, "need alpha >= 0, rho > 0, n_outer >= 1, n_cg >= 1");
+  if (p->prm.filter != LAM_FILTER_NONE || p->prm.input != LAM_INPUT_F32 || p->prm.pad_u || p->prm.spectral_alpha != 0.f)
+    return fail(p, LAM_EINVAL, "lam_admm_tv needs a plan with filter none, fp32 input, no padding, no spectral multiplier (L^T must be the plain adjoint)");
+  cudaSetDevice(p->device);
+  if (!is_device_ptr(proj) || !is_device_ptr(vol)) return fail(p, LAM_EUNSUPPORTED, "lam_admm_tv takes device pointers only");
+  if (p->spill) return fail(p, LAM_EUNSUPPORTED, "lam_admm_tv needs the in-core workspace (the plan runs the spilled schedule)");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const size_t nvox = (size_t)p->nz * p->n * p->n, nproj = (size_t)p->ntheta * p->h * p->w;
+  lam_status st;
+  if (!p->d_tv_g) {
+    if ((st = dalloc(p, &p->d_tv_g, nvox)) != LAM_OK) return st;
+    if ((st = dalloc(p, &p->d_tv_eta, nvox)) != LAM_OK) return st;
+    if ((st = dalloc(p, &p->d_tv_h, nvox)) != LAM_OK) return st;
+    if ((st = dalloc(p, &p->d_tv_psi, 3 * nvox)) != LAM_OK) return st;
+    if ((st = dalloc(p, &p->d_tv_lam, 3 * nvox)) != LAM_OK) return st;
+    if ((st = dalloc(p, &p->d_tv_r, nproj)) != LAM_OK) return st;
+    if ((st = dalloc(p, &p->d_tv_acc, 4)) != LAM_OK) return st;
+  }
+  const TvDims dims{p->n, p->nz};
+  const unsigned vb = (unsigned)((nvox + 255) / 256), rb = (unsigned)std::min<size_t>((nvox + 255) / 256, (size_t)p->n_sm * 16),
+                 pb = (unsigned)std::min<size_t>((nproj + 255) / 256, (size_t)p->n_sm * 16);
+  float *mu = vol, *g = p->d_tv_g, *eta = p->d_tv_eta, *hv = p->d_tv_h, *psi = p->d_tv_psi, *lamv = p->d_tv_lam, *r = p->d_tv_r;
+  long long launches = 0;
+  // three double sums per CG step, read back together
+  auto sums = [&](double out[4]) -> lam_status {
+    CU(p, cudaMemcpyAsync(out, p->d_tv_acc, 4 * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CU(p, cudaStreamSynchronize(s));
+    return LAM_OK;
+  };
+  CU(p, cudaMemsetAsync(mu, 0, nvox * 4, s));
+  CU(p, cudaMemsetAsync(psi, 0, 3 * nvox * 4, s));
+  CU(p, cudaMemsetAsync(lamv, 0, 3 * nvox * 4, s));
+  int hi = 0;
+  for (int k = 0; k < n_outer; ++k) {
+    // grad F(mu) = L^T (L mu - d) - rho div(grad mu - psi + lam / rho)                                   (Eq. 18)
+    if ((st = lam_forward(p, mu, r, s)) != LAM_OK) return st;
+    launches += p->launches;
+    k_axpby<<<pb, 256, 0, s>>>(r, 1.f, proj, -1.f, nproj);
+    if ((st = lam_backproject(p, r, g, s)) != LAM_OK) return st;
+    launches += p->launches;
+    k_tv_reggrad<<<vb, 256, 0, s>>>(mu, psi, lamv, rho, g, 1, dims);
+    CU(p, cudaMemsetAsync(eta, 0, nvox * 4, s));
+    k_axpby<<<rb, 256, 0, s>>>(eta, 0.f, g, -1.f, nvox);  // eta_0 = -grad F
+    launches += 3;
+    for (int m = 0; m < n_cg; ++m) {
+      // exact minimiser of the quadratic F along eta (reading Q19): gamma = -<g, eta> / (|L eta|^2 + rho |grad eta|^2)
+      if ((st = lam_forward(p, eta, r, s)) != LAM_OK) return st;
+      launches += p->launches;
+      CU(p, cudaMemsetAsync(p->d_tv_acc, 0, 4 * sizeof(double), s));
+      k_dot<<<pb, 256, 0, s>>>(r, r, nproj, p->d_tv_acc + 0);
+      k_tv_gradnorm2<<<rb, 256, 0, s>>>(eta, dims, p->d_tv_acc + 1);
+      k_dot<<<rb, 256, 0, s>>>(g, eta, nvox, p->d_tv_acc + 2);
+      double a[4];
+      if ((st = sums(a)) != LAM_OK) return st;
+      const double denom = a[0] + (double)rho * a[1];
+      if (!(denom > 0.0)) break;  // eta = 0: the subproblem is solved
+      const double gamma = -a[2] / denom;
+      k_axpby<<<rb, 256, 0, s>>>(mu, 1.f, eta, (float)gamma, nvox);
+      // H eta = L^T L eta - rho div grad eta;  grad F(mu + gamma eta) = grad F(mu) + gamma H eta  (F is quadratic)
+      if ((st = lam_backproject(p, r, hv, s)) != LAM_OK) return st;
+      launches += p->launches;
+      k_tv_reggrad<<<vb, 256, 0, s>>>(eta, nullptr, nullptr, rho, hv, 1, dims);
+      k_axpby<<<rb, 256, 0, s>>>(g, 1.f, hv, (float)gamma, nvox);
+      CU(p, cudaMemsetAsync(p->d_tv_acc, 0, 4 * sizeof(double), s));
+      k_dot<<<rb, 256, 0, s>>>(g, g, nvox, p->d_tv_acc + 0);
+      k_dot<<<rb, 256, 0, s>>>(hv, eta, nvox, p->d_tv_acc + 1);
+      if ((st = sums(a)) != LAM_OK) return st;
+      // Dai-Yuan: beta = |g_new|^2 / <g_new - g, eta> = |g_new|^2 / (gamma <H eta, eta>)                    (Eq. 19)
+      const double dy = gamma * a[1];
+      const double beta = dy != 0.0 ? a[0] / dy : 0.0;
+      k_axpby<<<rb, 256, 0, s>>>(eta, (float)beta, g, -1.f, nvox);
+      launches += 9;
+      if (history) history[hi++] = std::sqrt(a[0]);
+    }
+    k_tv_shrink<<<vb, 256, 0, s>>>(mu, psi, lamv, alpha, rho, dims);
+    launches += 1;
+  }
+  note_launch();
+  CU(p, cudaGetLastError());
+  if (g_launch_error != cudaSuccess) return fail(p, LAM_ECUDA, "kernel launch failed: %s", cudaGetErrorString(g_launch_error));
+  p->launches = launches;
   return LAM_OK;
 }
 

@@ -76,6 +76,7 @@ def lib():
     L.lam_backproject.argtypes = [P, P, P, P]
     L.lam_forward.argtypes = [P, P, P, P]
     L.lam_backproject_slice.argtypes = [P, P, C.c_int, C.c_int, C.POINTER(C.c_float), P, P]
+    L.lam_admm_tv.argtypes = [P, P, P, C.c_float, C.c_float, C.c_int, C.c_int, C.POINTER(C.c_double), P]
     L.lam_stage_ms.argtypes = [P, C.POINTER(C.c_float)]
     L.lam_set_profiling.argtypes = [P, C.c_int]
     L.lam_plan_info.argtypes = [P, C.POINTER(C.c_longlong)]
@@ -86,7 +87,7 @@ def lib():
 
 
 EXPORTS = ["lam_version", "lam_default_params", "lam_create", "lam_set_darkflat", "lam_backproject", "lam_forward",
-           "lam_backproject_slice",
+           "lam_backproject_slice", "lam_admm_tv",
            "lam_stage_ms", "lam_set_profiling", "lam_plan_info", "lam_last_error", "lam_destroy"]
 
 
@@ -133,6 +134,14 @@ def lam_backproject_slice(plan, proj_ptr, i3, centers, out_ptr, stream=0):
     nc = len(centers) if centers is not None else 0
     arr = (C.c_float * nc)(*[float(c) for c in centers]) if nc else None
     _check(lib().lam_backproject_slice(plan, C.c_void_p(proj_ptr), int(i3), nc, arr, C.c_void_p(out_ptr), C.c_void_p(stream)), plan)
+
+
+def lam_admm_tv(plan, proj_ptr, vol_ptr, alpha, rho, n_outer, n_cg, stream=0):
+    """Returns the list of ||grad F|| after every CG step (Appendix A)."""
+    hist = (C.c_double * (n_outer * n_cg))()
+    _check(lib().lam_admm_tv(plan, C.c_void_p(proj_ptr), C.c_void_p(vol_ptr), C.c_float(alpha), C.c_float(rho), int(n_outer),
+                             int(n_cg), hist, C.c_void_p(stream)), plan)
+    return list(hist)
 
 
 def lam_forward(plan, vol_ptr, proj_ptr, stream=0):
@@ -206,6 +215,17 @@ class Plan:
             stream = torch.cuda.current_stream().cuda_stream
         lam_backproject_slice(self._plan, proj.data_ptr(), i3, centers, out.data_ptr(), stream)
         return out
+
+    def admm_tv(self, proj, alpha, rho, n_outer, n_cg, vol=None, stream=None):
+        """TV-regularised reconstruction (Appendix A) -> (vol, ||grad F|| history)."""
+        import torch
+        assert proj.is_contiguous() and proj.dtype == torch.float32 and tuple(proj.shape) == (self.ntheta, self.h, self.w)
+        if vol is None:
+            vol = torch.empty((self.nz, self.n, self.n), dtype=torch.float32, device=proj.device)
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        hist = lam_admm_tv(self._plan, proj.data_ptr(), vol.data_ptr(), alpha, rho, n_outer, n_cg, stream)
+        return vol, hist
 
     def forward(self, vol, proj=None, stream=None):
         import torch

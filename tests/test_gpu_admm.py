@@ -1,0 +1,67 @@
+"""GPU parity of lam_admm_tv (Appendix A, Eqs. 10-20) against the fp64 oracle
+oracle/admm_tv.py, which runs the same iterations on the EXACT NUDFT pair (Eqs. 5, 7).  The GPU operators are the
+gridded lam_forward / lam_backproject (each ~1e-5 from the exact pair) in fp32; measured 4.7e-6 relative L2 on mu after
+3 x 3 iterations, gate 5e-5 (10x), ||grad F|| after every CG step within 1e-3."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import admm_tv as A
+from oracle import lam_oracle as O
+from paper_2401_11101_b200 import lam
+
+pytestmark = pytest.mark.gpu
+
+
+def _problem(seed=0):
+    n, nz, h, w, nth, phi = 32, 16, 32, 32, 12, 0.4
+    rng = np.random.default_rng(seed)
+    theta = np.linspace(0, 2 * np.pi, nth, endpoint=False)
+    g = O.Geometry(n, h, w, theta, phi, nz=nz, filter="none")
+    mu_true = np.zeros((nz, n, n))
+    mu_true[6:10, 10:22, 8:20] = 1.0
+    mu_true[7:9, 14:18, 22:27] = 0.5
+    d = O.forward_nudft(g, mu_true) + 0.05 * rng.normal(size=(nth, h, w))
+    return g, d.astype(np.float32), mu_true, (n, nz, h, w, theta, phi)
+
+
+def test_admm_tv_matches_the_oracle_iterations():
+    g, d, mu_true, (n, nz, h, w, theta, phi) = _problem()
+    alpha, rho, n_outer, n_cg = 0.3, 1.0, 3, 3
+    plan = lam.Plan(n, h, w, theta, phi, nz=nz, filter="none")
+    vol, hist = plan.admm_tv(torch.from_numpy(d).cuda(), alpha, rho, n_outer, n_cg)
+    torch.cuda.synchronize()
+    assert plan.info()["launches"] > 0
+    plan.close()
+    mu_ref, href = A.admm_tv(g, d.astype(np.float64), alpha, rho, n_outer, n_cg, track=False)
+    got = vol.cpu().numpy().astype(np.float64)
+    e = np.linalg.norm(got - mu_ref) / np.linalg.norm(mu_ref)
+    print("admm-tv mu vs oracle:", e, "||grad F|| gpu", hist, "oracle", href["gnorm_steps"])
+    assert e <= 5e-5, e
+    assert np.abs(got - mu_ref).max() <= 2e-4 * np.abs(mu_ref).max()
+    assert np.allclose(hist, href["gnorm_steps"], rtol=1e-3)
+
+
+def test_admm_tv_suppresses_noise_like_the_paper_says():
+    """PAPER.md:420 "noise suppression and incompleteness artefacts reduction": on noisy data the TV result has a lower
+    total variation and is closer to the piecewise-constant truth than unregularised least squares (alpha = 0)."""
+    g, d, mu_true, (n, nz, h, w, theta, phi) = _problem(1)
+    plan = lam.Plan(n, h, w, theta, phi, nz=nz, filter="none")
+    dd = torch.from_numpy(d).cuda()
+    tv_vol, _ = plan.admm_tv(dd, 0.4, 1.0, 10, 4)
+    tv_vol = tv_vol.cpu().numpy().astype(np.float64)
+    ls_vol, _ = plan.admm_tv(dd, 0.0, 1e-6, 1, 40)
+    ls_vol = ls_vol.cpu().numpy().astype(np.float64)
+    plan.close()
+    tv = lambda x: np.sqrt((A.grad(x) ** 2).sum(0)).sum()
+    assert tv(tv_vol) < 0.8 * tv(ls_vol)
+    assert np.linalg.norm(tv_vol - mu_true) < np.linalg.norm(ls_vol - mu_true)
+
+
+def test_admm_tv_rejects_a_filtered_plan():
+    g, d, mu_true, (n, nz, h, w, theta, phi) = _problem()
+    plan = lam.Plan(n, h, w, theta, phi, nz=nz)          # ramp filter: L^T would not be the adjoint
+    with pytest.raises(lam.LamError) as e:
+        plan.admm_tv(torch.from_numpy(d).cuda(), 0.1, 1.0, 1, 1)
+    assert e.value.status == lam.LAM_EINVAL
+    plan.close()
