@@ -20,11 +20,15 @@
 
 namespace lam {
 
+// Complex arithmetic on the packed fp32x2 pipe of sm_100a (FFMA2 / FMUL2 / FADD2: one issue slot per complex add, two
+// per complex product; ptxas folds the swap and the sign of (-a.y, a.x) into operand modifiers).  The FFT passes are
+// bound by instruction issue, not by the FMA pipe, so halving their floating-point instruction count is what counts.
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) {
-  return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+  const float2 t = __fmul2_rn(make_float2(-a.y, a.x), make_float2(b.y, b.y));  // (-a.y b.y, a.x b.y)
+  return __ffma2_rn(a, make_float2(b.x, b.x), t);                              // (a.x b.x - a.y b.y, a.y b.x + a.x b.y)
 }
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __ffma2_rn(b, make_float2(-1.f, -1.f), a); }
 
 template <int LOGN>
 struct FftShape {
@@ -105,7 +109,7 @@ __device__ __forceinline__ float2 rot16(float2 d, int k16) {
   if (k16 == 0) return d;
   if (k16 == 4) return DIR > 0 ? make_float2(-d.y, d.x) : make_float2(d.y, -d.x);
   float c = C[k16], s = DIR > 0 ? S[k16] : -S[k16];
-  return make_float2(fmaf(d.x, c, -d.y * s), fmaf(d.x, s, d.y * c));
+  return cmul(d, make_float2(c, s));
 }
 
 __host__ __device__ constexpr int brev_bits(int v, int bits) {

@@ -718,6 +718,8 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   auto tfast_lognb = [](int len, int lmax = 3) { int l = lmax; while (l > 0 && (size_t)(1 << l) * fft_tfast_pitch(len, 1 << l) * 8 > 200 * 1024) --l; return l; };
   p->cols_lcb = tfast_lognb(h);
   p->x2_lnb = tfast_lognb(M);
+  if (const char* e = getenv("LAM_TUNE_COLSLCB")) p->cols_lcb = std::min(p->cols_lcb, std::max(1, atoi(e)));
+  if (const char* e = getenv("LAM_TUNE_X2LNB")) p->x2_lnb = std::min(p->x2_lnb, std::max(1, atoi(e)));
   if (n % 8) return bail(fail(p, LAM_EUNSUPPORTED, "n must be a multiple of 8"));
   // x3 stage: 8 columns per block, fewer when that would leave one block per SM (>= 2 blocks of <= 100 KB)
   p->z_lcb = 3;

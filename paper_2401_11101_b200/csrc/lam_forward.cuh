@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(512) k_fft_x2_T(IfftArgs a) {
 
 // (k_ifft_x1)^T: G^T[pl][i2][i1] = sum_{kept k} e^{-2 pi i k i1/M} (-1)^k T^T[pl][i2][ix(k)]
 template <int LOGM>
-__global__ void __launch_bounds__(256) k_fft_x1_T(IfftArgs a) {
+__global__ void __launch_bounds__(256, 4) k_fft_x1_T(IfftArgs a) {
   constexpr int M = 1 << LOGM, P = fft_span(M);
   extern __shared__ float2 sm[];
   const int pl = blockIdx.y, r0 = blockIdx.x * a.nb;

@@ -308,7 +308,7 @@ struct ZArgs {
 __host__ __device__ constexpr int z_pitch(int cb) { return cb >= 8 ? cb + 4 : cb; }
 
 template <int LOGM3>
-__global__ void __launch_bounds__(512) k_zstage(ZArgs a) {
+__global__ void __launch_bounds__(512, 2) k_zstage(ZArgs a) {
   constexpr int M3 = 1 << LOGM3;
   const int zlog = a.lcb, zcb = 1 << a.lcb, P = fft_tfast_pitch(M3, zcb >> 1), PA = z_pitch(zcb);
   extern __shared__ float2 sm[];
