@@ -10,6 +10,7 @@ Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
   roofline  the dominant kernel group against its binding ceiling, plus `stages`: every stage against the HBM roofline
   cpu_baseline / --impl reference: the CPU fp64 oracle (oracle/), as it stands, on a bounded sample of the same workload
   all_configs  configs[2] and configs[4] (host-resident, PCIe inside) measured in the same run, with their stage tables
+  next_rows    lam_forward, lam_backproject_slice and lam_admm_tv timed on configs[2]
 N > 1: the path does not shard without an exchange step: N independent replicas, weak scaling.
 """
 import argparse
@@ -260,6 +261,50 @@ def measure(idx, steps, warmup, world, barrier, want_e2e=True, want_overlap=Fals
     return res
 
 
+def measure_next_rows(idx, reps=3):
+    """SURVEY.md 8(f) rows timed on one config (fp32 input): lam_forward, one lam_backproject_slice centre, one CG step of
+    lam_admm_tv.  CUDA events on the launching stream; not part of `value`."""
+    import torch
+    from paper_2401_11101_b200 import inputs, lam
+    cfg = inputs.config(idx)
+    plan = lam.Plan(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample, filter="none")
+    vol = torch.rand((cfg.nz, cfg.n, cfg.n), device="cuda")
+    proj = torch.empty((cfg.ntheta, cfg.h, cfg.w), device="cuda")
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def timed(fn, k):
+        fn()
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(k):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / k
+
+    out = {"workload": f"{cfg.name}: volume {cfg.n}x{cfg.n}x{cfg.nz}, {cfg.ntheta} angles, detector {cfg.h}x{cfg.w} fp32"}
+    t = timed(lambda: plan.forward(vol, proj), reps)
+    out["lam_forward"] = {"ms": round(t, 3), "GVoxel_per_s": round(cfg.voxels / t / 1e6, 3)}
+    centers = [cfg.w / 2 - 1.0, cfg.w / 2, cfg.w / 2 + 1.0]
+    sl = torch.empty((3, cfg.n, cfg.n), device="cuda")
+    t3 = timed(lambda: plan.backproject_slice(proj, cfg.nz // 2, centers, sl), 1)
+    t1 = timed(lambda: plan.backproject_slice(proj, cfg.nz // 2, centers[:1], sl[:1]), 1)
+    out["lam_backproject_slice"] = {"ms_first_centre": round(t1, 3), "ms_per_further_centre": round((t3 - t1) / 2, 3)}
+    t_a = time.perf_counter()
+    plan.admm_tv(proj, 0.1, 1.0, 1, 2, vol)
+    torch.cuda.synchronize()
+    t2 = (time.perf_counter() - t_a) * 1e3
+    t_a = time.perf_counter()
+    plan.admm_tv(proj, 0.1, 1.0, 1, 4, vol)
+    torch.cuda.synchronize()
+    t4 = (time.perf_counter() - t_a) * 1e3
+    out["lam_admm_tv"] = {"ms_per_cg_step": round((t4 - t2) / 2, 3), "note": "one lam_forward + one lam_backproject + TV kernels and reductions per step"}
+    plan.close()
+    del vol, proj, sl
+    torch.cuda.empty_cache()
+    return out
+
+
 def stage_report(cfg, stage, hbm):
     model = stage_model(cfg)
     out = {}
@@ -338,6 +383,13 @@ def run_ours(args):
             except Exception as e:  # a config that does not fit this box must not void the headline line
                 others[f"configs[{idx}]"] = {"error": str(e)[:200]}
                 torch.cuda.empty_cache()
+    next_rows = None
+    if world == 1 and not args.no_all_configs:
+        try:
+            next_rows = measure_next_rows(2)
+        except Exception as e:
+            next_rows = {"error": str(e)[:200]}
+            torch.cuda.empty_cache()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -390,6 +442,8 @@ def run_ours(args):
         out["overlap"] = r["overlap"]
     if others:
         out["all_configs"] = others
+    if next_rows:
+        out["next_rows"] = next_rows
     if not args.no_cpu_baseline:
         cb = cpu_sample(cfg)
         out["cpu_baseline"] = {"value": float(f"{cb['value']:.6g}"), "unit": UNIT, "cores": cb["cores"], "kind": "oracle",

@@ -167,7 +167,7 @@ const char* lam_last_error(const lam_plan* plan);
 
 void lam_destroy(lam_plan* plan);
 
-/* Library version string, e.g. "lam-b200 0.2 (sm_100a)". */
+/* Library version string, e.g. "lam-b200 0.3 (sm_100a)". */
 const char* lam_version(void);
 
 #ifdef __cplusplus

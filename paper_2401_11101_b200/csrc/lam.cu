@@ -621,7 +621,7 @@ void setup_ztma(lam_plan* p) {
 // ====================================================================================================================
 extern "C" {
 
-const char* lam_version(void) { return "lam-b200 0.2 (sm_100a)"; }
+const char* lam_version(void) { return "lam-b200 0.3 (sm_100a)"; }
 
 void lam_default_params(lam_params* p) {
   if (!p) return;

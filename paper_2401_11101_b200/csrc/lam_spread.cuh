@@ -460,7 +460,7 @@ __global__ void __launch_bounds__(32 * kSW, kSW == 1 ? 20 : 6) k_spread(SpreadAr
                     es.y = jj == j ? eo[j].y : es.y;
                   }
                   const float wM = fmaf(j1 < W / 2 ? dM : -dM, es.y, es.x);
-                  vw = make_float2(v.x * wM, v.y * wM);
+                  vw = __fmul2_rn(v, make_float2(wM, wM));
                   const int r0 = (int)(signed char)(pk & 0xffu);
                   addr = mycol_addr + (unsigned)(r0 * (kTS * 8));
                   rm = ok ? pk >> 8 : 0u;
@@ -477,10 +477,7 @@ __global__ void __launch_bounds__(32 * kSW, kSW == 1 ? 20 : 6) k_spread(SpreadAr
                     const bool last = i + 1 >= NI;
                     if (!last) prep(i + 1, nvw, nwm, naddr, nrm);
 #pragma unroll
-                    for (int j = 0; j < W; ++j) {
-                      c[j].x = fmaf(vw.x, wm[j], c[j].x);
-                      c[j].y = fmaf(vw.y, wm[j], c[j].y);
-                    }
+                    for (int j = 0; j < W; ++j) c[j] = __ffma2_rn(vw, make_float2(wm[j], wm[j]), c[j]);
                     static_for<0, W>([&](auto J) {
                       if (rm >> J.value & 1u) sts_f2<j_off(J.value)>(addr, c[J.value]);
                     });
@@ -506,10 +503,7 @@ __global__ void __launch_bounds__(32 * kSW, kSW == 1 ? 20 : 6) k_spread(SpreadAr
                       if (rm >> J.value & 1u) c[J.value] = lds_f2<j_off(J.value)>(addr);
                     });
 #pragma unroll
-                    for (int j = 0; j < W; ++j) {
-                      c[j].x = fmaf(vw.x, wm[j], c[j].x);
-                      c[j].y = fmaf(vw.y, wm[j], c[j].y);
-                    }
+                    for (int j = 0; j < W; ++j) c[j] = __ffma2_rn(vw, make_float2(wm[j], wm[j]), c[j]);
                     static_for<0, W>([&](auto J) {
                       if (rm >> J.value & 1u) sts_f2<j_off(J.value)>(addr, c[J.value]);
                     });
