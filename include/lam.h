@@ -31,13 +31,23 @@
  * copy streams that overlap the compute stream (Figs. 6-7: three streams, 2 + 2 buffers).  There
  * is no plan-owned pinned host staging: PINNED caller buffers (cudaHostAlloc / cudaHostRegister / torch pin_memory)
  * give asynchronous, overlapped copies; PAGEABLE buffers are accepted and give the same result, but the CUDA runtime
- * then stages every copy through its own bounce buffer and the copies do not overlap the kernels.  Every
- * intermediate of the path stays in device memory: the plan's workspace must fit params.device_bytes whatever the
- * pointer kinds are.  The caller owns proj and vol; the plan owns every workspace.
+ * then stages every copy through its own bounce buffer and the copies do not overlap the kernels.
+ *
+ * Workspace: params.device_bytes decides the schedule (PAPER.md:172 "> 64 GB for 2048^3", :181-191).  When the in-core
+ * workspace (all intermediates in device memory) fits the budget, it is used, whatever the pointer kinds are.  When it
+ * does not, lam_create plans the SPILLED schedule instead of failing: the projection spectra exist for one band of k_v
+ * planes at a time (the filter/FFT stage runs once per band over every projection), the cropped intermediate planes
+ * leave for a plan-owned PINNED HOST store ((h/2+1) n^2 complex64, reported by lam_plan_info; LAM_ENOMEM_HOST if it
+ * cannot be allocated) as they are produced and come back per slab of x2 rows for the x3 stage, all double-buffered on
+ * the copy streams.  lam_backproject gives the same result either way (to fp32 rounding); lam_forward,
+ * lam_backproject_slice and lam_admm_tv need the in-core workspace (LAM_EUNSUPPORTED on a spilled plan).  A budget too
+ * small even for one plane batch of every buffer gives LAM_ENOMEM_DEVICE.
+ * The caller owns proj and vol; the plan owns every workspace.
  *
  * All work of lam_backproject / lam_forward is enqueued on `cuda_stream` (a cudaStream_t, may be NULL = the
  * legacy default stream) and on plan-owned streams forked from / joined to it with events; the calls return
- * without synchronising when both pointers are device pointers.  With a host proj the call returns after the last
+ * without synchronising when both pointers are device pointers and the plan is in core (a spilled plan returns when
+ * its last copy has finished).  With a host proj the call returns after the last
  * host->device copy has completed (the caller may reuse proj), with a host vol after the last device->host copy
  * (vol is complete on return).
  *
@@ -59,8 +69,8 @@ typedef struct lam_plan lam_plan; /* opaque; owns all device/host workspace */
 typedef enum {
   LAM_OK = 0,
   LAM_EINVAL = 1,        /* bad argument (see lam_last_error)                              */
-  LAM_ENOMEM_DEVICE = 2, /* workspace does not fit params.device_bytes / free device memory */
-  LAM_ENOMEM_HOST = 3,   /* host allocation of the plan object failed                       */
+  LAM_ENOMEM_DEVICE = 2, /* not even the spilled schedule fits params.device_bytes / a cudaMalloc failed */
+  LAM_ENOMEM_HOST = 3,   /* host allocation failed: the plan object, or the pinned store of a spilled plan */
   LAM_ECUDA = 4,         /* CUDA runtime error, or no device                                */
   LAM_EUNSUPPORTED = 5   /* valid request outside what this build implements                */
 } lam_status;
@@ -80,7 +90,8 @@ typedef struct {
   float center_u;      /* rotation-axis column on the detector, pixels; NaN -> w/2                          */
   float center_v;      /* detector row hit by the ray through the origin; NaN -> h/2                        */
   float t_min;         /* transmission clamp before -log; 0 -> 1e-6                                         */
-  size_t device_bytes; /* workspace budget; 0 -> 90 % of the free device memory at lam_create               */
+  size_t device_bytes; /* workspace budget; 0 -> 90 % of the free device memory at lam_create; decides in-core
+                          against spilled schedule (header comment)                                        */
   int plane_batch;     /* k_v planes gridded + transformed per launch; 0 -> as many as fit 4 GB of fine grid  */
   int theta_chunk;     /* projections per filter/FFT launch (and per host->device copy); 0 -> auto          */
   int pad_u;           /* 1: every detector row is extended to 2w samples by replicating its edge values before the
@@ -158,7 +169,8 @@ lam_status lam_set_profiling(lam_plan* plan, int on);
 
 /* Workspace facts of a plan, for benchmarks and tests:
  * info[0] device bytes allocated, info[1] k_v planes, info[2] plane batch, info[3] gridding work items (jobs),
- * info[4] 1 if the last lam_backproject streamed through host pointers, info[5] theta chunk,
+ * info[4] bit 0: the last lam_backproject streamed through host pointers, bit 1: the plan runs the spilled schedule,
+ * info[5] theta chunk,
  * info[6] kernel launches of the last lam_backproject, info[7] pinned host bytes. */
 lam_status lam_plan_info(const lam_plan* plan, long long info[8]);
 

@@ -565,10 +565,14 @@ void setup_ztma(lam_plan* p) {
     }
     if (const char* e = getenv("LAM_TUNE_ZTHREADS")) p->z_threads = std::min(512, atoi(e));
   }
-  // The TMA-pipelined persistent form (k_zstage_tma) is kept for reference: measured SLOWER than the plain kernel
-  // (configs[2] 4.06 against 3.68 ms, configs[3] 60 against 44 ms), so it is opt-in.
+  // The TMA-pipelined persistent form (k_zstage_tma) is the default when the tensor map can be encoded and the plan is
+  // in core: measured at parity or slightly ahead of the plain kernel at equal columns per block (configs[2], 16
+  // columns: 3.25 against 3.29 ms; configs[3], 8 columns: 36.5 against 37.3 ms).  LAM_TUNE_ZTMA=0
+  // selects the plain kernel.
+  // Not for sigma*nz >= 2048 (configs[4]: 279 against 219 ms: its gridding phase splits every cell's band over two lanes,
+  // which costs more than the prefetch saves when the FFT is that long).
   const char* ez = getenv("LAM_TUNE_ZTMA");
-  if (!ez || atoi(ez) == 0 || p->spill) return;
+  if ((ez && atoi(ez) == 0) || p->spill || (p->M3 > 1024 && !ez)) return;
   typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -579,15 +583,12 @@ void setup_ztma(lam_plan* p) {
     cudaGetLastError();
     return;
   }
-  // columns per block: the largest of 8, 4, 2 whose double buffer lets two blocks share an SM, else the largest that fits
-  int lcb = 3, lmax = 3;
-  if (const char* e = getenv("LAM_TUNE_ZLCB")) lcb = lmax = std::max(1, std::min(4, atoi(e)));
+  // columns per block: the most of 16, 8, 4, 2 whose double buffer fits one SM (one persistent block per SM then; wider
+  // rows beat a second resident block, as for the plain kernel)
+  int lcb = (p->n % 16 == 0) ? 4 : 3;
+  if (const char* e = getenv("LAM_TUNE_ZLCB")) lcb = std::max(1, std::min(4, atoi(e)));
   int nbox, pbox, be;
-  while (lcb > 1 && ztma_smem(p, 1 << lcb, &nbox, &pbox, &be) > 112 * 1024) --lcb;
-  if (ztma_smem(p, 1 << lcb, &nbox, &pbox, &be) > 112 * 1024) {
-    lcb = lmax;
-    while (lcb > 1 && ztma_smem(p, 1 << lcb, &nbox, &pbox, &be) > 226 * 1024) --lcb;
-  }
+  while (lcb > 1 && ztma_smem(p, 1 << lcb, &nbox, &pbox, &be) > 226 * 1024) --lcb;
   const size_t sm = ztma_smem(p, 1 << lcb, &nbox, &pbox, &be);
   if (sm > 226 * 1024 || (p->n % (1 << lcb)) != 0) return;
   const int cb = 1 << lcb;
@@ -722,8 +723,13 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   if (const char* e = getenv("LAM_TUNE_X2LNB")) p->x2_lnb = std::min(p->x2_lnb, std::max(1, atoi(e)));
   if (n % 8) return bail(fail(p, LAM_EUNSUPPORTED, "n must be a multiple of 8"));
   // x3 stage: 8 columns per block, fewer when that would leave one block per SM (>= 2 blocks of <= 100 KB)
+  // x3 stage, columns per block.  Measured (configs[2], [3]): 16 columns when two blocks still share an SM (128-byte rows,
+  // conflict-free: S4 3.8 -> 3.3 ms), else 8 columns even at one block per SM (configs[3]: 35.0 ms against 41.8 ms with
+  // 4 columns and two blocks), else 4 or 2.
   p->z_lcb = 3;
-  while (p->z_lcb > 1 && zstage_smem(p, 1 << p->z_lcb) > 100 * 1024) --p->z_lcb;
+  if (n % 16 == 0 && zstage_smem(p, 16) <= 112 * 1024) p->z_lcb = 4;
+  while (p->z_lcb > 1 && zstage_smem(p, 1 << p->z_lcb) > 220 * 1024) --p->z_lcb;
+  if (const char* e = getenv("LAM_TUNE_ZLCB")) p->z_lcb = std::max(1, std::min(4, atoi(e)));
   if (zstage_smem(p, 1 << p->z_lcb) > 220 * 1024) return bail(fail(p, LAM_EUNSUPPORTED, "x3 stage does not fit shared memory (h = %d, sigma*nz = %d)", h, M3));
   // workspace: batch sizes from the budget
   size_t freeb = 0, totalb = 0;
@@ -1220,10 +1226,12 @@ lam_status lam_forward(lam_plan* p, const float* vol, float* proj, void* cuda_st
       DISPATCH_LOG(p->logM, x1T(dim3(M / p->x1_nb, nq), (size_t)p->x1_nb * fft_span(M) * sizeof(float2), s, a1));
       p->launches += 2;
     }
-    GatherArgs ga{p->geom, p->kp, p->d_G, p->d_S, p->WQ, p0, np};
+    const int b = p0 / p->PB;
+    GatherArgs ga{p->geom, p->kp, p->d_jobs + p->job_off[b], p->d_G, p->d_S, p->WQ, p0};
+    const long long njobs = p->job_off[b + 1] - p->job_off[b];
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;
-      k_gather<W><<<dim3((p->w + 1 + 255) / 256, p->ntheta, np), 256, 0, s>>>(ga);
+      k_gather<W><<<(unsigned)njobs, 32, gather_smem<W>(), s>>>(ga);
       note_launch();
     });
     p->launches += 1;

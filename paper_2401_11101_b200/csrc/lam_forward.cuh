@@ -1,12 +1,12 @@
 // lam_forward.cuh — kernels of lam_forward: proj = L vol, the exact transpose (over the reals) of lam_backproject
 // with filter = none, stage by stage in reverse order (Eq. 5: L = F*_2D F_u3D; the USFFT steps of
 // PAPER.md:136-138 in their forward order: division by the kernel transform, FFT, convolution-type interpolation).
-// Not tuned: it exists for the adjoint identity <L f, d> = <f, L* d> and as the forward model of iterative schemes.
+// It serves the adjoint identity <L f, d> = <f, L* d> and is the forward model of lam_admm_tv.
 //
 //   k_zstage_T   (x3 stage)^T    vol * deapodisation -> zero-pad -> forward FFT along x3 -> interpolate at t3(k_v)
 //   k_fft_x2_T   (k_ifft_x2)^T   zero-pad x2 (with the centring signs) -> forward FFT
 //   k_fft_x1_T   (k_ifft_x1)^T   zero-pad x1 -> forward FFT                     -> fine-grid plane G^T
-//   k_gather     (k_spread)^T    S^T[p][theta][q] = sum of W x W taps of G^T at the sample position (Eq. 6)
+//   k_gather     (k_spread)^T    S^T[p][theta][q] = sum of W x W taps of G^T at the sample position (Eq. 6), tile-staged
 //   k_cols_T     (k_cols)^T      un-fold the k_v >= 0 planes onto all h rows, inverse FFT along v
 //   k_rows_T     (k_rows)^T      conj(Pu) * half spectrum -> inverse FFT along u -> real part
 //
@@ -101,46 +101,99 @@ __global__ void __launch_bounds__(256, 4) k_fft_x1_T(IfftArgs a) {
   block_fft<LOGM, -1, false, true>(sm, a.nb, 0, P, a.tw, ld, st);
 }
 
-// (k_spread)^T: one thread per sample (theta, q) of plane p; the same positions, taps and periodic wrap as the
-// spreading (Eq. 6 times M; taps ceil(t - W/2) .. + W - 1; index (m + M/2) mod M)
+// (k_spread)^T, tile-staged: the transpose of the gridding reads W x W cells of the fine-grid plane per sample.  The same
+// work lists as k_spread are used (job = tile of plane p + the ranges of theta whose lines cross it): one warp stages the
+// tile with its W - 1 halo on the high side in shared memory (coalesced rows of G^T, periodic wrap), clips every line of
+// its ranges against the tile and lets lane = sample gather the samples whose FIRST tap cell lies inside the tile.  That
+// cell comes from the absolute position in double, by the same formula in every tile, so every sample is owned by exactly
+// one tile: plain stores, no atomics, and S^T needs no zeroing.  (The one-thread-per-sample form read its 36 taps from
+// L2: 30 of the 57 ms of lam_forward on configs[2].)
 struct GatherArgs {
   SpreadGeom g;
   KerPoly kp;
+  const Job* jobs;   // the k_spread work list of this plane batch
   const float2* G;   // [planes in batch][M][M]
   float2* S;         // [h/2+1][ntheta][WQ]
-  int WQ, p0, np;
+  int WQ, p0;
 };
 
 template <int W>
-__global__ void __launch_bounds__(256) k_gather(GatherArgs a) {
+__host__ __device__ constexpr int gather_pitch() { return ((kTS + W - 1) | 1); }  // odd pitch: rows start in different banks
+template <int W>
+__host__ __device__ constexpr size_t gather_smem() { return (size_t)(kTS + W - 1) * gather_pitch<W>() * sizeof(float2); }
+
+template <int W>
+__global__ void __launch_bounds__(32, 16) k_gather(GatherArgs a) {
+  constexpr int TH = kTS + W - 1, TP = gather_pitch<W>();
+  extern __shared__ float2 tile[];  // [TH][TP]
   const SpreadGeom& g = a.g;
-  const int q = blockIdx.x * blockDim.x + threadIdx.x, th = blockIdx.y, pl = blockIdx.z;
-  if (q > g.w) return;
-  const int p = a.p0 + pl, kv = p == g.hh ? -g.hh : p, ku = q - g.w / 2;
-  const double2 cs = g.cs[th];
-  const double rho = g.rho_unit * kv, u = (double)g.a1 * ku;
-  const double t1d = u * cs.x + rho * cs.y, t2d = u * cs.y - rho * cs.x;
-  const double c1 = ceil(t1d - 0.5 * W), c2 = ceil(t2d - 0.5 * W);
-  float w1[W], w2[W];
-  kernel_weights<W>(a.kp, (float)(t1d - c1 - (0.5 * W - 0.5)), w1);
-  kernel_weights<W>(a.kp, (float)(t2d - c2 - (0.5 * W - 0.5)), w2);
-  const int M = g.M, m1 = (int)c1 + M / 2, m2 = (int)c2 + M / 2;
-  const float2* Gp = a.G + (size_t)pl * M * M;
-  float2 acc = make_float2(0.f, 0.f);
-#pragma unroll
-  for (int j2 = 0; j2 < W; ++j2) {
-    const float2* row = Gp + (size_t)((m2 + j2) & (M - 1)) * M;
-    float2 r = make_float2(0.f, 0.f);
-#pragma unroll
-    for (int j1 = 0; j1 < W; ++j1) {
-      const float2 v = row[(m1 + j1) & (M - 1)];
-      r.x = fmaf(v.x, w1[j1], r.x);
-      r.y = fmaf(v.y, w1[j1], r.y);
+  const int lane = threadIdx.x;
+  const Job jb = a.jobs[blockIdx.x];
+  const int tx = jb.w[0] & 0xff, ty = (jb.w[0] >> 8) & 0xff, p = (jb.w[0] >> 16) & 0x1fff;
+  const int usex = jb.w[1] & 7, usey = (jb.w[1] >> 3) & 7, nranges = (jb.w[1] >> 6) & 7;
+  if (nranges == 0) return;  // untouched tile: owns no sample
+  const int kv = p == g.hh ? -g.hh : p;
+  const double rho = g.rho_unit * kv;
+  const int M = g.M, hw = g.w / 2;
+  const int mx0 = tx * kTS - M / 2, my0 = ty * kTS - M / 2;
+  {
+    const float2* Gp = a.G + (size_t)(p - a.p0) * M * M;
+    for (int i = lane; i < TH * TH; i += 32) {
+      const int r = i / TH, c = i - r * TH;
+      tile[r * TP + c] = __ldg(Gp + (size_t)((ty * kTS + r) & (M - 1)) * M + ((tx * kTS + c) & (M - 1)));
     }
-    acc.x = fmaf(r.x, w2[j2], acc.x);
-    acc.y = fmaf(r.y, w2[j2], acc.y);
   }
-  a.S[((size_t)p * g.ntheta + th) * a.WQ + q] = acc;
+  __syncwarp();
+  float2* Sp = a.S + (size_t)p * g.ntheta * a.WQ;
+#pragma unroll 1
+  for (int ri = 0; ri < nranges; ++ri) {
+    const unsigned rw = jb.w[2 + ri];
+    const int rs = rw & 0x3fff, rend = rs + (int)((rw >> 14) & 0x7ff);
+    for (int tb = rs; tb < rend; tb += 32) {
+      const int th = tb + lane;
+      const bool tvalid = th < rend;
+      const double2 cs = tvalid ? g.cs[th] : make_double2(1.0, 0.0);
+#pragma unroll 1
+      for (int sy = -1; sy <= 1; ++sy) {
+        if (!(usey >> (sy + 1) & 1)) continue;
+        const float oy = (float)(-rho * cs.x - my0 + (double)sy * M);
+#pragma unroll 1
+        for (int sx = -1; sx <= 1; ++sx) {
+          if (!(usex >> (sx + 1) & 1)) continue;
+          const float ox = (float)(rho * cs.y - mx0 + (double)sx * M);
+          int ka = 1, kb = 0;
+          if (tvalid) clip_box<W>(ox, oy, (float)cs.x, (float)cs.y, g.a1, hw, kTS, kTS, ka, kb);
+          unsigned mask = __ballot_sync(0xffffffffu, ka <= kb);
+          while (mask) {
+            const int cur = __ffs(mask) - 1;
+            mask &= mask - 1;
+            const int thc = tb + cur, kac = __shfl_sync(0xffffffffu, ka, cur), kbc = __shfl_sync(0xffffffffu, kb, cur);
+            const double cx = __shfl_sync(0xffffffffu, cs.x, cur), sn = __shfl_sync(0xffffffffu, cs.y, cur);
+            for (int k = kac + lane; k <= kbc; k += 32) {
+              const double u = (double)g.a1 * k;
+              const double t1d = u * cx + rho * sn, t2d = u * sn - rho * cx;
+              const double c1 = ceil(t1d - 0.5 * W), c2 = ceil(t2d - 0.5 * W);
+              const int lx = ((int)c1 - mx0) & (M - 1), ly = ((int)c2 - my0) & (M - 1);
+              if (lx >= kTS || ly >= kTS) continue;  // another tile owns this sample
+              float w1[W], w2[W];
+              kernel_weights<W>(a.kp, (float)(t1d - c1 - (0.5 * W - 0.5)), w1);
+              kernel_weights<W>(a.kp, (float)(t2d - c2 - (0.5 * W - 0.5)), w2);
+              const float2* t0 = tile + ly * TP + lx;
+              float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+              for (int j2 = 0; j2 < W; ++j2) {
+                float2 r = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int j1 = 0; j1 < W; ++j1) r = __ffma2_rn(t0[j2 * TP + j1], make_float2(w1[j1], w1[j1]), r);
+                acc = __ffma2_rn(r, make_float2(w2[j2], w2[j2]), acc);
+              }
+              Sp[(size_t)thc * a.WQ + hw + k] = acc;
+            }
+          }
+        }
+      }
+    }
+  }
 }
 
 // (k_cols)^T: for column k_u = k >= 0 of projection theta, C^T[p], p = 0..h-1, from the planes 0..h/2:

@@ -305,7 +305,7 @@ struct ZArgs {
 
 // row pitch of the staged planes in float2: rows two or three planes apart (neighbouring cells) land in different
 // 16-byte bank groups for the 128-bit reads of phase 2
-__host__ __device__ constexpr int z_pitch(int cb) { return cb >= 8 ? cb + 4 : cb; }
+__host__ __device__ constexpr int z_pitch(int cb) { return cb == 8 ? cb + 4 : cb; }  // 16 columns: one 128-byte row per quarter-warp, no padding needed
 
 template <int LOGM3>
 __global__ void __launch_bounds__(512, 2) k_zstage(ZArgs a) {
