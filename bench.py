@@ -465,7 +465,8 @@ def run_reference(args):
     vals, secs, last = [], [], None
     for it in range(args.warmup + args.steps):
         t0 = time.perf_counter()
-        last = cpu_sample(cfg, nangles=args.cpu_angles or None, mult=2)
+        # 13 samples at the default --steps 10 --warmup 3: one and two angles on a 2-slice slab keep a step near 10 s
+        last = cpu_sample(cfg, nangles=args.cpu_angles or 1, slab=2, mult=2)
         if it >= args.warmup:
             vals.append(last["value"])
             secs.append(time.perf_counter() - t0)

@@ -596,8 +596,12 @@ void setup_ztma(lam_plan* p) {
   cuuint64_t gstr[2] = {(cuuint64_t)p->n * 8, (cuuint64_t)p->n * p->n * 8};
   cuuint32_t box[3] = {(cuuint32_t)cb, 1, (cuuint32_t)pbox};
   cuuint32_t estr[3] = {1, 1, 1};
+  // L2 promotion no wider than a box row: with 128-byte promotion the 64-byte rows of an 8-column box fetched 1.7x the
+  // algorithmic bytes from DRAM (ncu, configs[3]: 58 GB for 34 GB)
+  const CUtensorMapL2promotion promo = cb >= 16 ? CU_TENSOR_MAP_L2_PROMOTION_L2_128B
+                                       : cb >= 8 ? CU_TENSOR_MAP_L2_PROMOTION_L2_64B : CU_TENSOR_MAP_L2_PROMOTION_NONE;
   CUresult r = ((encode_fn)fn)(&p->tmapA, CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, (void*)p->d_A, gdim, gstr, box, estr,
-                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
                                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return;
   // block size: fewest wasted lanes over the rounds of phase 2 (nact * 8 tasks), 384..640 threads
