@@ -729,9 +729,11 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   // x3 stage: 8 columns per block, fewer when that would leave one block per SM (>= 2 blocks of <= 100 KB)
   // x3 stage, columns per block.  Measured (configs[2], [3]): 16 columns when two blocks still share an SM (128-byte rows,
   // conflict-free: S4 3.8 -> 3.3 ms), else 8 columns even at one block per SM (configs[3]: 35.0 ms against 41.8 ms with
-  // 4 columns and two blocks), else 4 or 2.
+  // 4 columns and two blocks) up to sigma*nz = 1024; for longer transforms 4 columns and two blocks (configs[4]: 219
+  // against 299 ms), else whatever fits.
   p->z_lcb = 3;
   if (n % 16 == 0 && zstage_smem(p, 16) <= 112 * 1024) p->z_lcb = 4;
+  else if (zstage_smem(p, 8) > 112 * 1024 && M3 > 1024 && zstage_smem(p, 4) <= 112 * 1024) p->z_lcb = 2;  // configs[4]: 219 against 299 ms
   while (p->z_lcb > 1 && zstage_smem(p, 1 << p->z_lcb) > 220 * 1024) --p->z_lcb;
   if (const char* e = getenv("LAM_TUNE_ZLCB")) p->z_lcb = std::max(1, std::min(4, atoi(e)));
   if (zstage_smem(p, 1 << p->z_lcb) > 220 * 1024) return bail(fail(p, LAM_EUNSUPPORTED, "x3 stage does not fit shared memory (h = %d, sigma*nz = %d)", h, M3));
@@ -888,7 +890,8 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s, bool slic
     }
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;
-      const size_t sm = spread_smem();
+      size_t sm = spread_smem();
+      if (const char* e = getenv("LAM_TUNE_SPREAD_PAD")) sm += (size_t)atoi(e);  // occupancy experiment: fewer resident warps
       cudaFuncSetAttribute(k_spread<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
       k_spread<W><<<(unsigned)sa.njobs, 32 * kSW, sm, s>>>(sa);
       note_launch();
