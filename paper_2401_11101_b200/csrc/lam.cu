@@ -384,7 +384,8 @@ lam_status build_jobs(lam_plan* p) {
       p->multi_off[b] = (long long)multi.size();
       order.resize(i1 - i0);
       for (size_t i = 0; i < order.size(); ++i) order[i] = (unsigned)i;
-      std::stable_sort(order.begin(), order.end(), [&](unsigned x, unsigned y) { return lines[i0 + x] > lines[i0 + y]; });
+      std::stable_sort(order.begin(), order.end(),
+                       [&](unsigned x, unsigned y) { return (lines[i0 + x] & 0xffffffu) > (lines[i0 + y] & 0xffffffu); });  // top bits: image masks
       for (unsigned o : order) {
         const size_t i = i0 + o;
         offs[i] = (unsigned)tot;
@@ -405,6 +406,7 @@ lam_status build_jobs(lam_plan* p) {
     const int np = std::min(chunk, NP - p0);
     cudaMemcpy(d_off, offs.data() + (size_t)p0 * ntiles, (size_t)np * ntiles * 4, cudaMemcpyHostToDevice);
     cudaMemcpy(d_count, counts.data() + (size_t)p0 * ntiles, (size_t)np * ntiles * 4, cudaMemcpyHostToDevice);
+    cudaMemcpy(d_lines, lines.data() + (size_t)p0 * ntiles, (size_t)np * ntiles * 4, cudaMemcpyHostToDevice);
     launch(p0, np, true);
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) st = fail(p, LAM_ECUDA, "work-list fill pass: %s", cudaGetErrorString(e));

@@ -124,7 +124,7 @@ struct JobsArgs {
   SpreadGeom g;
   int p0, np;             // planes [p0, p0+np)
   unsigned* count;        // [np][nt*nt] jobs per tile (count pass: out; fill pass: in)
-  unsigned* lines;        // [np][nt*nt] lines crossing the tile (count pass: out)
+  unsigned* lines;        // [np][nt*nt] lines crossing the tile (count pass: out); bits 24..29: periodic images in use
   const unsigned* off;    // [np][nt*nt] first job of the tile in `jobs` (fill pass)
   Job* jobs;              // fill pass
 };
@@ -160,9 +160,14 @@ __global__ void k_jobs(JobsArgs a) {
     }
     return any;
   };
-  // pass A: which images are ever hit (all jobs of the tile carry the same masks)
-  int usex = 0, usey = 0;
-  for (int th = 0; th < g.ntheta; ++th) crosses(th, candx, candy, usex, usey);
+  // which periodic images are ever hit (all jobs of the tile carry the same masks): the count pass tests every candidate
+  // image and records the union in the top bits of `lines`; the fill pass reads it back and tests only those
+  int usex = candx, usey = candy, seenx = 0, seeny = 0;
+  if (FILL) {
+    const unsigned m = a.lines[gid] >> 24;
+    usex = m & 7;
+    usey = (m >> 3) & 7;
+  }
   // pass B: ranges of one orientation each, packed into jobs
   const unsigned total = FILL ? a.count[gid] : 0;
   Job* out = FILL ? a.jobs + a.off[gid] : nullptr;
@@ -193,8 +198,7 @@ __global__ void k_jobs(JobsArgs a) {
     for (int th = 0; th < g.ntheta; ++th) {
       const double2 cs = g.cs[th];
       const int o = fabsf((float)cs.x) >= fabsf((float)cs.y) ? 0 : 1;
-      int dx = 0, dy = 0;
-      const bool hit = crosses(th, usex, usey, dx, dy);
+      const bool hit = crosses(th, usex, usey, seenx, seeny);
       if (rs >= 0 && (o != ro || (!hit && th - rlast > kRangeGap))) close_range();
       if (hit) {
         if (rs < 0) { rs = th; ro = o; }
@@ -209,7 +213,7 @@ __global__ void k_jobs(JobsArgs a) {
     if (nr > 0) emit_job();
   }
   if (njobs == 0) emit_job();  // untouched tile: one job without ranges stores zeros
-  if (!FILL) { a.count[gid] = njobs; a.lines[gid] = nlines; }
+  if (!FILL) { a.count[gid] = njobs; a.lines[gid] = nlines | (unsigned)(seenx | seeny << 3) << 24; }
 }
 
 struct SpreadArgs {
