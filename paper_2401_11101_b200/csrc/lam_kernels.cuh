@@ -38,7 +38,7 @@ struct RowsArgs {
 };
 
 template <int LOGW, bool RAW>
-__global__ void __launch_bounds__(256) k_rows(RowsArgs a) {
+__global__ void __launch_bounds__(256, 4) k_rows(RowsArgs a) {
   constexpr int w = 1 << LOGW, P = fft_span(w);
   extern __shared__ float2 sm[];
   const int th = blockIdx.y, pair0 = blockIdx.x * a.nb;
