@@ -52,3 +52,30 @@ def test_random_configurations_against_exact_columns(seed):
         assert e <= TOL[Wk], f"{what}: rel L2 {e:.3e} > {TOL[Wk]:.0e}"
         worst = max(worst, e / TOL[Wk])
     print(f"seed {seed}: worst error / gate = {worst:.2f}")
+
+
+@pytest.mark.parametrize("seed", [11, 12])
+def test_random_configurations_adjoint_identity(seed):
+    """<L f, d> = <f, L* d> ("adjoint") on random shapes: lam_forward (tile-staged gather on the k_spread work
+    lists) against lam_backproject with filter none, random f and d, relative 2e-5 (fp32 sums of ~1e6 terms)."""
+    rng = np.random.default_rng(seed)
+    for it in range(10):
+        n = int(rng.choice([32, 64, 128]))
+        nz = int(rng.choice([16, 32, 64]))
+        h = int(rng.choice([32, 64, 128, 256]))
+        w = int(rng.choice([32, 64, 128, 256]))
+        nth = int(rng.choice([1, 3, 40, 257, 400]))
+        phi = float(rng.uniform(0, math.radians(60)))
+        theta = rng.uniform(0, 2 * np.pi, nth) if rng.random() < 0.5 else np.linspace(0, 2 * np.pi, nth, endpoint=False)
+        Wk = int(rng.choice([4, 6, 8]))
+        cu = w / 2 + (float(rng.uniform(-3, 3)) if rng.random() < 0.5 else 0.0)
+        plan = lam.Plan(n, h, w, theta, phi, nz=nz, filter="none", width=Wk, center_u=cu, plane_batch=int(rng.choice([0, 2])))
+        f = torch.from_numpy(rng.normal(size=(nz, n, n)).astype(np.float32)).cuda()
+        d = torch.from_numpy(rng.normal(size=(nth, h, w)).astype(np.float32)).cuda()
+        Lf = plan.forward(f)
+        LTd = plan.backproject(d)
+        plan.close()
+        a = float((Lf.double() * d.double()).sum())
+        b = float((f.double() * LTd.double()).sum())
+        scale = float(Lf.double().norm() * d.double().norm())
+        assert abs(a - b) <= 2e-5 * scale, f"seed {seed} case {it}: n={n} nz={nz} h={h} w={w} nth={nth} W={Wk}: {a} vs {b} (scale {scale})"
