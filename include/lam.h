@@ -137,7 +137,8 @@ lam_status lam_backproject_slice(lam_plan* plan, const void* proj, int i3, int n
 /* proj <- L vol (overwrites proj, float32): Eq. 5 as the exact transpose, stage by stage in reverse
  * order, of lam_backproject with filter none (the plan's filter setting is ignored; an input plan of type uint16
  * still yields float32 line integrals).  Device pointers only (host pointers: LAM_EUNSUPPORTED); asynchronous on
- * cuda_stream.  <L f, d> = <f, L* d> holds to fp32 rounding (about 1e-6 relative).  Not tuned. */
+ * cuda_stream.  <L f, d> = <f, L* d> holds to fp32 rounding (about 1e-6 relative).  Needs the
+ * in-core workspace (LAM_EUNSUPPORTED on a spilled plan).  About the cost of one lam_backproject. */
 lam_status lam_forward(lam_plan* plan, const float* vol, float* proj, void* cuda_stream);
 
 /* TV-regularised reconstruction of PAPER.md Appendix A (Eqs. 10-20):
