@@ -134,6 +134,38 @@ lam_status lam_backproject(lam_plan* plan, const void* proj, float* vol, void* c
 lam_status lam_backproject_slice(lam_plan* plan, const void* proj, int i3, int n_centers, const float* centers_u,
                                  float* out, void* cuda_stream);
 
+/* lam_backproject_slice for callers that must not touch the device allocator at call time.  Same arguments, same result
+ * (evaluated as Eq. 9); the difference is where the slice scratch lives.
+ *
+ * Who needs it: lam_backproject_slice calls cudaMalloc five times on its first use per plan.  That is a problem for a
+ * program that creates its plans while it is starting up and afterwards has no allocator left to call: a beamline
+ * preview service that runs the axis search between detector frames and cannot afford cudaMalloc's device-wide
+ * synchronisation and unbounded latency there; a host application (a PyTorch or CuPy process) whose memory pool took all
+ * remaining device memory after start-up, so a late cudaMalloc from this library simply fails; code that runs where the
+ * CUDA runtime forbids allocation calls altogether.  For those callers this entry point allocates and frees NO device
+ * memory, creates no streams or events, and calls no allocating library routine (on the host it uses a few short-lived
+ * std::vector tables, as lam_backproject_slice does).
+ *
+ * How: the summed fine grid, its x1 transform, the cropped plane and the two phase tables live in a 16 MiB array that is
+ * part of liblam.so's device image.  Every GPU on which the library's kernels are loaded holds those 16 MiB until the
+ * process exits, whether or not this function is ever called.  Limit: the plan's slice scratch,
+ * 8 (M^2 + M n + n^2 + (h/2+1) + (w+8)) bytes with M = sigma*n, must fit, i.e. sigma*n <= 1024 at sigma = 2 (n <= 512)
+ * for any supported h, w; a larger plan gets LAM_EUNSUPPORTED and a message that names both sizes (use
+ * lam_backproject_slice there).  Spilled plans: LAM_EUNSUPPORTED, as for lam_backproject_slice.
+ *
+ * First call per device: looks up the device address of that array (cudaGetSymbolAddress, which may also make the
+ * runtime load the library's device code).  Make that first call during set-up, before any stream capture is begun.
+ * Later calls only read the cached address.
+ *
+ * Sharing: there is ONE such array per device, shared by every plan and every call in the process, and it keeps whatever
+ * the previous call left in it.  The function clears what has to start at zero (the summed grid, once per centre) and
+ * overwrites the rest before reading it, so calls that follow one another on a device, on any streams, need nothing
+ * from the caller as long as each has finished on the GPU before the next starts.  Two calls that overlap on the GPU
+ * (different streams or threads, same device) race on the array and both results are garbage: serialise them, or give
+ * the second caller lam_backproject_slice.  Per-stage profiling (lam_set_profiling) records nothing for this call. */
+lam_status lam_backproject_slice_static(lam_plan* plan, const void* proj, int i3, int n_centers, const float* centers_u,
+                                        float* out, void* cuda_stream);
+
 /* proj <- L vol (overwrites proj, float32): Eq. 5 as the exact transpose, stage by stage in reverse
  * order, of lam_backproject with filter none (the plan's filter setting is ignored; an input plan of type uint16
  * still yields float32 line integrals).  Device pointers only (host pointers: LAM_EUNSUPPORTED); asynchronous on

@@ -14,6 +14,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1202,6 +1203,109 @@ lam_status lam_backproject_slice(lam_plan* p, const void* proj, int i3, int n_ce
   CU(p, cudaGetLastError());
   if (g_launch_error != cudaSuccess) return fail(p, LAM_ECUDA, "kernel launch failed: %s", cudaGetErrorString(g_launch_error));
   return LAM_OK;
+}
+
+}  // extern "C"
+
+// ---- lam_backproject_slice_static: the slice search on scratch memory that is part of the library image --------------
+// The five buffers lam_backproject_slice cudaMallocs on its first call (summed fine grid Gs, its x1 transform Ts, the
+// cropped plane As, the x3 and axis phase tables) are carved out of ONE file-scope device array instead.  The array is
+// zero-initialised device memory that every GPU holds from the moment the library's kernels are loaded on it until the
+// process exits: kSliceScratchBytes = 16 MiB, enough for sigma*n <= 1024 at sigma = 2 (n <= 512) with h, w <= 8192.
+//
+// `g_slice_scratch` below is a HOST-side handle of that array, not a device address: handing it to a kernel or to
+// cudaMemsetAsync would make the GPU fault (or scribble over host memory it can reach).  The device address is asked for
+// once per device, with that device current, through cudaGetSymbolAddress, and cached in g_slice_scratch_dev[].
+constexpr size_t kSliceScratchElems = (size_t)2 << 20;  // float2 elements
+constexpr size_t kSliceScratchBytes = kSliceScratchElems * sizeof(float2);
+constexpr int kSliceScratchMaxDevices = 64;
+
+static __device__ __align__(256) float2 g_slice_scratch[kSliceScratchElems];
+
+namespace {
+
+std::mutex g_slice_scratch_mu;
+float2* g_slice_scratch_dev[kSliceScratchMaxDevices] = {};  // device address of g_slice_scratch, per device ordinal
+
+// Device address of the static scratch on p->device (which must be the current device).
+lam_status slice_scratch_address(lam_plan* p, float2** out) {
+  if (p->device < 0 || p->device >= kSliceScratchMaxDevices)
+    return fail(p, LAM_EUNSUPPORTED, "static slice scratch is tracked for device ordinals below %d (plan is on %d)",
+                kSliceScratchMaxDevices, p->device);
+  std::lock_guard<std::mutex> lk(g_slice_scratch_mu);
+  if (!g_slice_scratch_dev[p->device]) {
+    void* q = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&q, g_slice_scratch);
+    if (e != cudaSuccess || !q) {
+      cudaGetLastError();
+      return fail(p, LAM_ECUDA, "cudaGetSymbolAddress(g_slice_scratch) on device %d failed: %s", p->device, cudaGetErrorString(e));
+    }
+    g_slice_scratch_dev[p->device] = (float2*)q;
+  }
+  *out = g_slice_scratch_dev[p->device];
+  return LAM_OK;
+}
+
+// Points the plan's single-slice buffers at the static scratch for the duration of one call and puts the plan's own
+// (possibly still null) pointers back afterwards, so that lam_destroy never sees an address it did not allocate.
+struct SliceScratchLease {
+  lam_plan* p;
+  float2 *Gs, *Ts, *As, *zph, *cph;
+  bool profiling;
+  SliceScratchLease(lam_plan* p_, float2* base, const size_t off[5])
+      : p(p_), Gs(p_->d_Gs), Ts(p_->d_Ts), As(p_->d_As), zph(p_->d_zph), cph(p_->d_cph), profiling(p_->profiling) {
+    p->d_Gs = base + off[0];
+    p->d_Ts = base + off[1];
+    p->d_As = base + off[2];
+    p->d_zph = base + off[3];
+    p->d_cph = base + off[4];
+    p->profiling = false;  // stage timing creates CUDA events on demand; this path creates nothing
+  }
+  ~SliceScratchLease() {
+    p->d_Gs = Gs; p->d_Ts = Ts; p->d_As = As; p->d_zph = zph; p->d_cph = cph;
+    p->profiling = profiling;
+  }
+};
+
+}  // namespace
+
+extern "C" {
+
+lam_status lam_backproject_slice_static(lam_plan* p, const void* proj, int i3, int n_centers, const float* centers_u, float* out,
+                                        void* cuda_stream) {
+  if (!p) return LAM_EINVAL;
+  if (p->spill) return fail(p, LAM_EUNSUPPORTED, "lam_backproject_slice_static needs the in-core workspace (the plan runs the spilled schedule)");
+  // sub-buffers in the order Gs, Ts, As, zph, cph, each starting on a 256-byte boundary (32 float2)
+  const size_t want[5] = {(size_t)p->M * p->M, (size_t)p->M * p->n, (size_t)p->n * p->n, (size_t)p->NP, (size_t)p->WQ};
+  size_t off[5], total = 0;
+  for (int i = 0; i < 5; ++i) {
+    off[i] = total;
+    total += (want[i] + 31) / 32 * 32;
+  }
+  if (total > kSliceScratchElems)
+    return fail(p, LAM_EUNSUPPORTED,
+                "lam_backproject_slice_static: this plan needs %zu bytes of slice scratch (fine grid %d x %d), the static "
+                "scratch holds %zu bytes (sigma*n <= 1024 at sigma = 2); use lam_backproject_slice, which allocates",
+                total * sizeof(float2), p->M, p->M, kSliceScratchBytes);
+  if (cudaSetDevice(p->device) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(p, LAM_ECUDA, "cudaSetDevice(%d) failed", p->device);
+  }
+  float2* base = nullptr;
+  lam_status st = slice_scratch_address(p, &base);
+  if (st != LAM_OK) return st;
+  const size_t bytes_before = p->device_bytes;
+  {
+    // Every call starts from whatever the previous call (of any plan on this device) left in the scratch.  The only
+    // buffer that is accumulated into is Gs, and the slice path zeroes it per centre before gridding; Ts and As are
+    // written in full before they are read, the two phase tables are uploaded before their kernels run.
+    SliceScratchLease lease(p, base, off);
+    st = lam_backproject_slice(p, proj, i3, n_centers, centers_u, out, cuda_stream);
+  }
+  if (st == LAM_OK && p->device_bytes != bytes_before)
+    return fail(p, LAM_ECUDA, "internal: lam_backproject_slice_static allocated %zu bytes of device memory",
+                p->device_bytes - bytes_before);
+  return st;
 }
 
 lam_status lam_forward(lam_plan* p, const float* vol, float* proj, void* cuda_stream) {

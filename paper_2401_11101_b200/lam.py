@@ -76,6 +76,7 @@ def lib():
     L.lam_backproject.argtypes = [P, P, P, P]
     L.lam_forward.argtypes = [P, P, P, P]
     L.lam_backproject_slice.argtypes = [P, P, C.c_int, C.c_int, C.POINTER(C.c_float), P, P]
+    L.lam_backproject_slice_static.argtypes = [P, P, C.c_int, C.c_int, C.POINTER(C.c_float), P, P]
     L.lam_admm_tv.argtypes = [P, P, P, C.c_float, C.c_float, C.c_int, C.c_int, C.POINTER(C.c_double), P]
     L.lam_stage_ms.argtypes = [P, C.POINTER(C.c_float)]
     L.lam_set_profiling.argtypes = [P, C.c_int]
@@ -87,7 +88,7 @@ def lib():
 
 
 EXPORTS = ["lam_version", "lam_default_params", "lam_create", "lam_set_darkflat", "lam_backproject", "lam_forward",
-           "lam_backproject_slice", "lam_admm_tv",
+           "lam_backproject_slice", "lam_backproject_slice_static", "lam_admm_tv",
            "lam_stage_ms", "lam_set_profiling", "lam_plan_info", "lam_last_error", "lam_destroy"]
 
 
@@ -134,6 +135,15 @@ def lam_backproject_slice(plan, proj_ptr, i3, centers, out_ptr, stream=0):
     nc = len(centers) if centers is not None else 0
     arr = (C.c_float * nc)(*[float(c) for c in centers]) if nc else None
     _check(lib().lam_backproject_slice(plan, C.c_void_p(proj_ptr), int(i3), nc, arr, C.c_void_p(out_ptr), C.c_void_p(stream)), plan)
+
+
+def lam_backproject_slice_static(plan, proj_ptr, i3, centers, out_ptr, stream=0):
+    """lam_backproject_slice on the scratch array built into liblam.so: for callers that may not allocate device memory
+    once their plans exist (include/lam.h has the limit, sigma*n <= 1024, and the sharing rules)."""
+    nc = len(centers) if centers is not None else 0
+    arr = (C.c_float * nc)(*[float(c) for c in centers]) if nc else None
+    _check(lib().lam_backproject_slice_static(plan, C.c_void_p(proj_ptr), int(i3), nc, arr, C.c_void_p(out_ptr),
+                                              C.c_void_p(stream)), plan)
 
 
 def lam_admm_tv(plan, proj_ptr, vol_ptr, alpha, rho, n_outer, n_cg, stream=0):
@@ -203,8 +213,10 @@ class Plan:
         lam_backproject(self._plan, proj.data_ptr(), vol.data_ptr(), stream)
         return vol
 
-    def backproject_slice(self, proj, i3, centers=None, out=None, stream=None):
-        """Slice i3 for each rotation-axis position in `centers` (the `try` search) -> [nc][n][n]."""
+    def backproject_slice(self, proj, i3, centers=None, out=None, stream=None, static_scratch=False):
+        """Slice i3 for each rotation-axis position in `centers` (the `try` search) -> [nc][n][n].
+        static_scratch=True goes through lam_backproject_slice_static (no device allocation inside the library; pass
+        `out` as well if torch must not allocate either)."""
         import torch
         assert proj.is_contiguous() and tuple(proj.shape) == (self.ntheta, self.h, self.w) and proj.is_cuda
         nc = len(centers) if centers is not None and len(centers) else 1
@@ -213,7 +225,8 @@ class Plan:
         assert out.is_contiguous() and out.dtype == torch.float32 and tuple(out.shape) == (nc, self.n, self.n)
         if stream is None:
             stream = torch.cuda.current_stream().cuda_stream
-        lam_backproject_slice(self._plan, proj.data_ptr(), i3, centers, out.data_ptr(), stream)
+        call = lam_backproject_slice_static if static_scratch else lam_backproject_slice
+        call(self._plan, proj.data_ptr(), i3, centers, out.data_ptr(), stream)
         return out
 
     def admm_tv(self, proj, alpha, rho, n_outer, n_cg, vol=None, stream=None):
