@@ -201,6 +201,9 @@ __global__ void k_jobs(JobsArgs a) {
       const bool hit = crosses(th, usex, usey, seenx, seeny);
       if (rs >= 0 && (o != ro || (!hit && th - rlast > kRangeGap))) close_range();
       if (hit) {
+        // a range may span up to kRangeGap misses between hits, so the length is checked BEFORE the hit is appended:
+        // a length past the 11-bit field would spill into the ydom bit
+        if (rs >= 0 && th + 1 - rs > kRangeMaxLen) close_range();
         if (rs < 0) { rs = th; ro = o; }
         rlast = th;
         ++jl;
