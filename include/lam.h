@@ -47,7 +47,8 @@
  * All work of lam_backproject / lam_forward is enqueued on `cuda_stream` (a cudaStream_t, may be NULL = the
  * legacy default stream) and on plan-owned streams forked from / joined to it with events; the calls return
  * without synchronising when both pointers are device pointers and the plan is in core (a spilled plan returns when
- * its last copy has finished).  With a host proj the call returns after the last
+ * all of the call's work has finished on the device: its plan-owned pinned store and slab buffers are then free for
+ * the next call, on whatever stream that is issued).  With a host proj the call returns after the last
  * host->device copy has completed (the caller may reuse proj), with a host vol after the last device->host copy
  * (vol is complete on return).
  *
@@ -91,7 +92,10 @@ typedef struct {
   float center_v;      /* detector row hit by the ray through the origin; NaN -> h/2                        */
   float t_min;         /* transmission clamp before -log; 0 -> 1e-6                                         */
   size_t device_bytes; /* workspace budget; 0 -> 90 % of the free device memory at lam_create; decides in-core
-                          against spilled schedule (header comment)                                        */
+                          against spilled schedule (header comment).  It covers what lam_create allocates.  Outside
+                          it, allocated on first use: the host-pointer staging (2 theta chunks of input + 2 output
+                          slabs), the slice buffers of lam_backproject_slice (8 (M^2 + M n + n^2) bytes) and the
+                          lam_admm_tv workspace (9 volumes + 1 projection set); leave room for the ones you use   */
   int plane_batch;     /* k_v planes gridded + transformed per launch; 0 -> as many as fit 4 GB of fine grid  */
   int theta_chunk;     /* projections per filter/FFT launch (and per host->device copy); 0 -> auto          */
   int pad_u;           /* 1: every detector row is extended to 2w samples by replicating its edge values before the
@@ -184,7 +188,9 @@ lam_status lam_forward(lam_plan* plan, const float* vol, float* proj, void* cuda
  * L = lam_forward, L^T = lam_backproject of THIS plan, which must have been created with LAM_FILTER_NONE, fp32 input,
  * no padding and no spectral multiplier (else LAM_EINVAL).  grad: forward differences, zero at the far faces.
  * proj: the data d, [n_theta][h][w] float32; vol: the result mu (overwritten); both DEVICE pointers.
- * history: NULL, or a HOST array of n_outer * n_cg doubles that receives ||grad F|| after every CG step.
+ * history: NULL, or a HOST array of n_outer * n_cg doubles; entry k*n_cg + m receives ||grad F|| after CG step m of
+ * outer iteration k.  When a direction has no curvature left (the subproblem is solved early), the remaining entries of
+ * that outer iteration repeat the last norm taken.  NaN or Inf in proj: LAM_EINVAL at the first step that sees it.
  * The call synchronises cuda_stream twice per CG step (the step lengths are host scalars). */
 lam_status lam_admm_tv(lam_plan* plan, const float* proj, float* vol, float alpha, float rho, int n_outer, int n_cg,
                        double* history, void* cuda_stream);

@@ -794,10 +794,11 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
     for (int i = 0; i < 2; ++i) {
       if ((st = dalloc(p, &p->d_Ab[i], (size_t)p->PB * aplane)) != LAM_OK) return bail(st);
       if ((st = dalloc(p, &p->d_As2[i], (size_t)p->NP * p->ZRs * n)) != LAM_OK) return bail(st);
-      cudaEventCreateWithFlags(&p->ev_ab_ready[i], cudaEventDisableTiming);
-      cudaEventCreateWithFlags(&p->ev_ab_free[i], cudaEventDisableTiming);
-      cudaEventCreateWithFlags(&p->ev_sl_ready[i], cudaEventDisableTiming);
-      cudaEventCreateWithFlags(&p->ev_sl_free[i], cudaEventDisableTiming);
+      for (cudaEvent_t* ev : {&p->ev_ab_ready[i], &p->ev_ab_free[i], &p->ev_sl_ready[i], &p->ev_sl_free[i]})
+        if (cudaEventCreateWithFlags(ev, cudaEventDisableTiming) != cudaSuccess) {
+          *ev = nullptr;
+          return bail(fail(p, LAM_ECUDA, "spilled schedule: cudaEventCreateWithFlags failed: %s", cudaGetErrorString(cudaGetLastError())));
+        }
     }
     const size_t hbytes = (size_t)p->NP * aplane * 8;
     if (cudaHostAlloc((void**)&p->h_A, hbytes, cudaHostAllocDefault) != cudaSuccess) {
@@ -1125,7 +1126,13 @@ lam_status lam_backproject(lam_plan* p, const void* proj, float* vol, void* cuda
   if (g_launch_error != cudaSuccess) return fail(p, LAM_ECUDA, "kernel launch failed: %s", cudaGetErrorString(g_launch_error));
   p->stage_valid = p->profiling;
   p->last_call_host = !proj_dev || !vol_dev;
-  if (p->spill) CU(p, cudaStreamSynchronize(p->s_d2h));  // the pinned plane store is plan-owned: nothing of it is in flight on return
+  if (p->spill) {
+    // the pinned plane store and the slab buffers are plan-owned and shared by every later call, whatever stream it
+    // is given: nothing of them is in flight on return.  The x3 kernels on `s` wait for every slab read-back on s_h2d,
+    // so s_d2h + s cover all three streams.
+    CU(p, cudaStreamSynchronize(p->s_d2h));
+    CU(p, cudaStreamSynchronize(s));
+  }
   if (!proj_dev) CU(p, cudaStreamSynchronize(p->s_h2d));  // the caller's host projections are consumed on return
   if (!vol_dev) CU(p, cudaStreamSynchronize(p->s_d2h));   // host results are valid on return
   return LAM_OK;
@@ -1401,7 +1408,7 @@ lam_status lam_admm_tv(lam_plan* p, const float* proj, float* vol, float alpha, 
   CU(p, cudaMemsetAsync(mu, 0, nvox * 4, s));
   CU(p, cudaMemsetAsync(psi, 0, 3 * nvox * 4, s));
   CU(p, cudaMemsetAsync(lamv, 0, 3 * nvox * 4, s));
-  int hi = 0;
+  double gnorm = 0.0;  // ||grad F|| after the last CG step taken
   for (int k = 0; k < n_outer; ++k) {
     // grad F(mu) = L^T (L mu - d) - rho div(grad mu - psi + lam / rho)                                   (Eq. 18)
     if ((st = lam_forward(p, mu, r, s)) != LAM_OK) return st;
@@ -1424,7 +1431,14 @@ lam_status lam_admm_tv(lam_plan* p, const float* proj, float* vol, float alpha, 
       double a[4];
       if ((st = sums(a)) != LAM_OK) return st;
       const double denom = a[0] + (double)rho * a[1];
-      if (!(denom > 0.0)) break;  // eta = 0: the subproblem is solved
+      if (!std::isfinite(denom) || !std::isfinite(a[2]))
+        return fail(p, LAM_EINVAL, "lam_admm_tv: non-finite step length at outer iteration %d, CG step %d (NaN or Inf in proj?)", k, m);
+      if (!(denom > 0.0)) {
+        // eta = 0: the subproblem is solved.  The steps that are skipped still own their history slots (k n_cg + m).
+        if (history)
+          for (int q = m; q < n_cg; ++q) history[(size_t)k * n_cg + q] = gnorm;
+        break;
+      }
       const double gamma = -a[2] / denom;
       k_axpby<<<rb, 256, 0, s>>>(mu, 1.f, eta, (float)gamma, nvox);
       // H eta = L^T L eta - rho div grad eta;  grad F(mu + gamma eta) = grad F(mu) + gamma H eta  (F is quadratic)
@@ -1441,7 +1455,8 @@ lam_status lam_admm_tv(lam_plan* p, const float* proj, float* vol, float alpha, 
       const double beta = dy != 0.0 ? a[0] / dy : 0.0;
       k_axpby<<<rb, 256, 0, s>>>(eta, (float)beta, g, -1.f, nvox);
       launches += 9;
-      if (history) history[hi++] = std::sqrt(a[0]);
+      gnorm = std::sqrt(a[0]);
+      if (history) history[(size_t)k * n_cg + m] = gnorm;
     }
     k_tv_shrink<<<vb, 256, 0, s>>>(mu, psi, lamv, alpha, rho, dims);
     launches += 1;

@@ -65,3 +65,20 @@ def test_admm_tv_rejects_a_filtered_plan():
         plan.admm_tv(torch.from_numpy(d).cuda(), 0.1, 1.0, 1, 1)
     assert e.value.status == lam.LAM_EINVAL
     plan.close()
+
+
+def test_admm_tv_history_keeps_its_slots_when_cg_stops_early_and_nan_is_an_error():
+    """include/lam.h: history[k n_cg + m] belongs to CG step m of outer iteration k.  Zero data: the first direction has
+    no curvature (eta = 0), every step is skipped, every slot is still written (0) and mu stays 0.  NaN data: LAM_EINVAL."""
+    g, d, mu_true, (n, nz, h, w, theta, phi) = _problem()
+    plan = lam.Plan(n, h, w, theta, phi, nz=nz, filter="none")
+    vol, hist = plan.admm_tv(torch.zeros((len(theta), h, w), device="cuda"), 0.3, 1.0, 2, 3)
+    assert hist == [0.0] * 6 and float(vol.abs().max()) == 0.0
+    bad = torch.from_numpy(d).cuda()
+    bad[3, 5, 7] = float("nan")
+    with pytest.raises(lam.LamError) as e:
+        plan.admm_tv(bad, 0.3, 1.0, 2, 3)
+    assert e.value.status == lam.LAM_EINVAL and "non-finite" in str(e.value)
+    vol, hist = plan.admm_tv(torch.from_numpy(d).cuda(), 0.3, 1.0, 1, 2)     # the plan is still usable afterwards
+    assert len(hist) == 2 and all(np.isfinite(hist)) and min(hist) > 0.0
+    plan.close()
