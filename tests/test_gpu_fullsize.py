@@ -10,8 +10,10 @@ tile and batch) runs on a scan in which K RANDOM angles carry the generated raw 
 (a zero line integral, exactly, because the fixed-pattern fields are rounded to integers); the exact answer is the
 K-angle sum, which the oracle evaluates from the SAME uint16 + dark/flat arrays on 16 columns (path A) and two
 slices (C').  Only the filter's quadrature weight pi cos(phi)/N_theta (reading Q3) differs between a K-angle and an
-N_theta-angle geometry: the oracle's result is scaled by K/N_theta, stated here and nowhere hidden.  The angle subset
-changes from run to run (seed printed; LAM_TEST_SEED pins it); K/N_theta of the theta-dependent work lists carry data.
+N_theta-angle geometry: the oracle's result is scaled by K/N_theta, stated here and nowhere hidden.
+K = 450 of 1800 (25 %) for configs[3] in core and K = 128 of 3000 (4.3 %) for configs[4], on exact columns only (one C'
+slice at these K is ten minutes of oracle time); the spilled configs[3] run keeps K = 64 and its two C' slices.  The
+angle subset is drawn from SEED, a constant of this file (LAM_TEST_SEED overrides it), so a failure reproduces.
 """
 import os
 import time
@@ -26,7 +28,7 @@ from paper_2401_11101_b200 import inputs, lam
 from gates import L2_NOISY, L2_RAW_SPARSE, MAXABS_NOISY, NORTH_LARGE, check
 
 pytestmark = pytest.mark.gpu
-SEED = int(os.environ.get("LAM_TEST_SEED", str(int(time.time()) // 600)))
+SEED = int(os.environ.get("LAM_TEST_SEED", "20261106"))
 
 
 def random_columns(cfg, ncols, rng):
@@ -90,12 +92,12 @@ def sparse_raw_scan(cfg, K, rng, device):
     return full, sel, raw.cpu().numpy(), dark, flat
 
 
-def check_raw(cfg, vol, sel, raw_sel, dark, flat, rng, ncols=16, nslices=2):
+def check_raw(cfg, vol, sel, raw_sel, dark, flat, rng, ncols=16, nslices=2, l2=L2_RAW_SPARSE):
     K = len(sel)
     geom = O.Geometry(cfg.n, cfg.h, cfg.w, cfg.theta()[sel], cfg.phi, nz=cfg.nz, dark=dark.numpy(), flat=flat.numpy())
     cols = random_columns(cfg, ncols, rng)
     ref = O.fbp_nudft(geom, raw_sel, cols=cols) * (K / cfg.ntheta)
-    e = check(columns_of(vol, cols), ref, L2_RAW_SPARSE, MAXABS_NOISY, f"{cfg.name}: {ncols} exact columns (seed {SEED})")
+    e = check(columns_of(vol, cols), ref, l2, MAXABS_NOISY, f"{cfg.name}: {ncols} exact columns (seed {SEED})")
     msg = f"{ncols} exact columns rel L2 {e[0]:.3e} max-abs {e[1]:.3e}"
     colrms = float(np.sqrt(np.mean(ref ** 2)))
     for i3 in rng.choice(np.arange(cfg.nz // 4, 3 * cfg.nz // 4), size=nslices, replace=False):
@@ -113,7 +115,7 @@ def test_config3_full_size_raw_uint16():
     if free < 120e9:
         pytest.skip("configs[3] needs ~100 GB of device memory")
     rng = np.random.default_rng(SEED + 3)
-    K = 64
+    K = 450
     proj, sel, raw_sel, dark, flat = sparse_raw_scan(cfg, K, rng, "cuda")
     plan = lam.Plan(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample, input="u16")
     plan.set_darkflat(dark.cuda(), flat.cuda())
@@ -123,7 +125,7 @@ def test_config3_full_size_raw_uint16():
     plan.close()
     del proj
     torch.cuda.empty_cache()
-    msg = check_raw(cfg, vol, sel, raw_sel, dark, flat, rng)
+    msg = check_raw(cfg, vol, sel, raw_sel, dark, flat, rng, ncols=24, nslices=0, l2=L2_NOISY)
     print(f"configs[3] full size, data at {K} of {cfg.ntheta} random angles ({100.0 * K / cfg.ntheta:.1f} % of theta): {msg}; plan = {info}")
 
 
@@ -173,7 +175,7 @@ def test_config4_out_of_core_host_buffers():
     if free < 150e9 or psutil.virtual_memory().available < need_host + 30e9:
         pytest.skip("configs[4] needs ~145 GB of device memory and ~135 GB of host memory")
     rng = np.random.default_rng(SEED + 4)
-    K = 32
+    K = 128
     try:
         proj, sel, raw_sel, dark, flat = sparse_raw_scan(cfg, K, rng, "cpu")
         vol = torch.empty((cfg.nz, cfg.n, cfg.n), dtype=torch.float32, pin_memory=True)
@@ -188,6 +190,6 @@ def test_config4_out_of_core_host_buffers():
     info = plan.info()
     plan.close()
     del proj
-    msg = check_raw(cfg, vol, sel, raw_sel, dark, flat, rng)
+    msg = check_raw(cfg, vol, sel, raw_sel, dark, flat, rng, ncols=16, nslices=0)
     print(f"configs[4] out-of-core: {dt:.2f} s wall ({cfg.voxels / dt / 1e9:.2f} GVoxel/s incl. PCIe), data at {K} of "
           f"{cfg.ntheta} random angles ({100.0 * K / cfg.ntheta:.1f} % of theta): {msg}; plan = {info}")
