@@ -104,6 +104,12 @@ typedef struct {
   float spectral_alpha;/* alpha >= 0 of the 2-D low-pass 1/(1 + alpha ((k_u/w)^2 + (k_v/h)^2)) applied to every
                           projection spectrum: the single-distance Paganin multiplier named as pre-processing in
                           PAPER.md:199, 279, applied to the line integrals (reading Q17); 0: none                 */
+  int z_form;          /* form of the x3 stage: 0 -> the library's policy (TMA-fed persistent kernel below
+                          sigma*nz = 2048 on an in-core plan, plain kernel otherwise); 1: plain kernel; 2: TMA form
+                          wherever its tensor map and buffers can be set up (never on a spilled plan).  Both forms
+                          compute the same sums in a different order; tests compare them                          */
+  int z_columns;       /* x2-columns per block of the x3 stage: 0 -> policy; 2, 4, 8 or 16 (must divide n; reduced
+                          if the block would not fit shared memory)                                               */
 } lam_params;
 
 /* Fill *p with the defaults (KB, W = 6, sigma = 2, ramp filter, fp32 input, centred axis). */
@@ -218,7 +224,7 @@ const char* lam_last_error(const lam_plan* plan);
 
 void lam_destroy(lam_plan* plan);
 
-/* Library version string, e.g. "lam-b200 0.3 (sm_100a)". */
+/* Library version string, e.g. "lam-b200 0.4 (sm_100a)". */
 const char* lam_version(void);
 
 #ifdef __cplusplus

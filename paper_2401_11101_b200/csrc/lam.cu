@@ -566,16 +566,15 @@ void setup_ztma(lam_plan* p) {
       const long cost = (long)((total + T - 1) / T) * T;
       if (bestcost < 0 || cost < bestcost || (cost == bestcost && T > p->z_threads)) { bestcost = cost; p->z_threads = T; }
     }
-    if (const char* e = getenv("LAM_TUNE_ZTHREADS")) p->z_threads = std::min(512, atoi(e));
   }
   // The TMA-pipelined persistent form (k_zstage_tma) is the default when the tensor map can be encoded and the plan is
   // in core: measured at parity or slightly ahead of the plain kernel at equal columns per block (configs[2], 16
-  // columns: 3.25 against 3.29 ms; configs[3], 8 columns: 36.5 against 37.3 ms).  LAM_TUNE_ZTMA=0
+  // columns: 3.25 against 3.29 ms; configs[3], 8 columns: 36.5 against 37.3 ms).  params.z_form = 1
   // selects the plain kernel.
   // Not for sigma*nz >= 2048 (configs[4]: 279 against 219 ms: its gridding phase splits every cell's band over two lanes,
   // which costs more than the prefetch saves when the FFT is that long).
-  const char* ez = getenv("LAM_TUNE_ZTMA");
-  if ((ez && atoi(ez) == 0) || p->spill || (p->M3 > 1024 && !ez)) return;
+  const int form = p->prm.z_form;  // 0: this policy, 1: plain kernel, 2: TMA form wherever it can be set up
+  if (form == 1 || p->spill || (p->M3 > 1024 && form != 2)) return;
   typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -589,7 +588,7 @@ void setup_ztma(lam_plan* p) {
   // columns per block: the most of 16, 8, 4, 2 whose double buffer fits one SM (one persistent block per SM then; wider
   // rows beat a second resident block, as for the plain kernel)
   int lcb = (p->n % 16 == 0) ? 4 : 3;
-  if (const char* e = getenv("LAM_TUNE_ZLCB")) lcb = std::max(1, std::min(4, atoi(e)));
+  if (p->prm.z_columns) lcb = ilog2(p->prm.z_columns);
   int nbox, pbox, be;
   while (lcb > 1 && ztma_smem(p, 1 << lcb, &nbox, &pbox, &be) > 226 * 1024) --lcb;
   const size_t sm = ztma_smem(p, 1 << lcb, &nbox, &pbox, &be);
@@ -615,7 +614,6 @@ void setup_ztma(lam_plan* p) {
     const long cost = (long)((total + T - 1) / T) * T;
     if (bestcost < 0 || cost < bestcost || (cost == bestcost && T > best)) { bestcost = cost; best = T; }
   }
-  if (const char* e = getenv("LAM_TUNE_ZTHREADS")) best = atoi(e);
   int occ = 0;
   dispatch_log_impl<kLogMin>(p->logM3, [&](auto L_) { occ = decltype(L_)::ztma_occupancy(best, sm); });
   if (occ < 1) return;
@@ -629,7 +627,7 @@ void setup_ztma(lam_plan* p) {
 // ====================================================================================================================
 extern "C" {
 
-const char* lam_version(void) { return "lam-b200 0.3 (sm_100a)"; }
+const char* lam_version(void) { return "lam-b200 0.4 (sm_100a)"; }
 
 void lam_default_params(lam_params* p) {
   if (!p) return;
@@ -649,6 +647,8 @@ void lam_default_params(lam_params* p) {
   p->theta_chunk = 0;
   p->pad_u = 0;
   p->spectral_alpha = 0.f;
+  p->z_form = 0;
+  p->z_columns = 0;
 }
 
 const char* lam_last_error(const lam_plan* plan) { return plan ? plan->err.c_str() : g_create_error.c_str(); }
@@ -679,6 +679,10 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   if (P.filter < 0 || P.filter > 3) return fail(nullptr, LAM_EINVAL, "unknown filter");
   if (!(P.spectral_alpha >= 0.f)) return fail(nullptr, LAM_EINVAL, "spectral_alpha must be >= 0");
   if (P.pad_u != 0 && P.pad_u != 1) return fail(nullptr, LAM_EINVAL, "pad_u must be 0 or 1");
+  if (P.z_form < 0 || P.z_form > 2) return fail(nullptr, LAM_EINVAL, "z_form must be 0 (auto), 1 (plain kernel) or 2 (TMA form)");
+  if (P.z_columns != 0 && P.z_columns != 2 && P.z_columns != 4 && P.z_columns != 8 && P.z_columns != 16)
+    return fail(nullptr, LAM_EINVAL, "z_columns must be 0 (auto), 2, 4, 8 or 16");
+  if (P.z_columns && n % P.z_columns) return fail(nullptr, LAM_EINVAL, "z_columns must divide n");
   if (P.pad_u && w > 4096) return fail(nullptr, LAM_EUNSUPPORTED, "pad_u needs w <= 4096 (rows of 2w samples)");
   if (P.input != LAM_INPUT_F32 && P.input != LAM_INPUT_U16_RAW) return fail(nullptr, LAM_EINVAL, "unknown input type");
   if (P.width != 4 && P.width != 6 && P.width != 8) return fail(nullptr, LAM_EUNSUPPORTED, "width must be 4, 6 or 8");
@@ -726,8 +730,6 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   auto tfast_lognb = [](int len, int lmax = 3) { int l = lmax; while (l > 0 && (size_t)(1 << l) * fft_tfast_pitch(len, 1 << l) * 8 > 200 * 1024) --l; return l; };
   p->cols_lcb = tfast_lognb(h);
   p->x2_lnb = tfast_lognb(M);
-  if (const char* e = getenv("LAM_TUNE_COLSLCB")) p->cols_lcb = std::min(p->cols_lcb, std::max(1, atoi(e)));
-  if (const char* e = getenv("LAM_TUNE_X2LNB")) p->x2_lnb = std::min(p->x2_lnb, std::max(1, atoi(e)));
   if (n % 8) return bail(fail(p, LAM_EUNSUPPORTED, "n must be a multiple of 8"));
   // x3 stage: 8 columns per block, fewer when that would leave one block per SM (>= 2 blocks of <= 100 KB)
   // x3 stage, columns per block.  Measured (configs[2], [3]): 16 columns when two blocks still share an SM (128-byte rows,
@@ -738,7 +740,10 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   if (n % 16 == 0 && zstage_smem(p, 16) <= 112 * 1024) p->z_lcb = 4;
   else if (zstage_smem(p, 8) > 112 * 1024 && M3 > 1024 && zstage_smem(p, 4) <= 112 * 1024) p->z_lcb = 2;  // configs[4]: 219 against 299 ms
   while (p->z_lcb > 1 && zstage_smem(p, 1 << p->z_lcb) > 220 * 1024) --p->z_lcb;
-  if (const char* e = getenv("LAM_TUNE_ZLCB")) p->z_lcb = std::max(1, std::min(4, atoi(e)));
+  if (P.z_columns) {
+    p->z_lcb = ilog2(P.z_columns);
+    while (p->z_lcb > 1 && zstage_smem(p, 1 << p->z_lcb) > 220 * 1024) --p->z_lcb;
+  }
   if (zstage_smem(p, 1 << p->z_lcb) > 220 * 1024) return bail(fail(p, LAM_EUNSUPPORTED, "x3 stage does not fit shared memory (h = %d, sigma*nz = %d)", h, M3));
   // workspace: batch sizes from the budget
   size_t freeb = 0, totalb = 0;
@@ -758,11 +763,10 @@ lam_status lam_create(int n, int h, int w, int n_theta, float phi_rad, const flo
   // in L2 (1-4 planes) are SLOWER than whole batches (S3 13.7 / 11.6 / 11.1 ms at 1 / 2 / 4 planes against 9.7 ms): the
   // passes are issue-bound, not HBM-bound, and short launches pay their tails.  So T covers the whole plane batch.
   p->TSB = p->PB;
-  if (const char* e = getenv("LAM_TUNE_TSB")) p->TSB = std::max(1, std::min(p->PB, atoi(e)));
   // the gridding work lists are allocated by build_jobs: about one 32-byte job per (plane, tile)
   const size_t jobs_est = (size_t)((double)p->NP * (M / kTS) * (M / kTS) * 1.1) * sizeof(Job);
   const size_t need = (size_t)p->TC * rproj + arena * 8 + (size_t)p->PB * gplane + (size_t)p->TSB * tplane + jobs_est + p->device_bytes;
-  if (need <= budget && !getenv("LAM_TUNE_FORCE_SPILL")) {
+  if (need <= budget) {
     if ((st = dalloc(p, &p->d_R, (size_t)p->TC * h * p->WR)) != LAM_OK) return bail(st);
     if ((st = dalloc(p, &p->d_arena, arena)) != LAM_OK) return bail(st);
     p->d_A = p->d_arena;
@@ -895,7 +899,6 @@ static void launch_planes(lam_plan* p, int p0, int np, cudaStream_t s, bool slic
     dispatch_W(p->W, [&](auto Wc) {
       constexpr int W = decltype(Wc)::value;
       size_t sm = spread_smem();
-      if (const char* e = getenv("LAM_TUNE_SPREAD_PAD")) sm += (size_t)atoi(e);  // occupancy experiment: fewer resident warps
       cudaFuncSetAttribute(k_spread<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
       k_spread<W><<<(unsigned)sa.njobs, 32 * kSW, sm, s>>>(sa);
       note_launch();

@@ -30,7 +30,8 @@ class lam_params(C.Structure):
     _fields_ = [("nz", C.c_int), ("kernel", C.c_int), ("width", C.c_int), ("oversample", C.c_float),
                 ("shape", C.c_float), ("filter", C.c_int), ("input", C.c_int), ("center_u", C.c_float),
                 ("center_v", C.c_float), ("t_min", C.c_float), ("device_bytes", C.c_size_t),
-                ("plane_batch", C.c_int), ("theta_chunk", C.c_int), ("pad_u", C.c_int), ("spectral_alpha", C.c_float)]
+                ("plane_batch", C.c_int), ("theta_chunk", C.c_int), ("pad_u", C.c_int), ("spectral_alpha", C.c_float),
+                ("z_form", C.c_int), ("z_columns", C.c_int)]
 
 
 class LamError(RuntimeError):
@@ -183,7 +184,7 @@ def lam_destroy(plan):
 class Plan:
     def __init__(self, n, h, w, theta, phi, nz=None, kernel="kb", width=6, oversample=2.0, shape=0.0, filter="ramp",
                  input="f32", center_u=None, center_v=None, t_min=1e-6, device_bytes=0, plane_batch=0, theta_chunk=0,
-                 pad_u=False, spectral_alpha=0.0):
+                 pad_u=False, spectral_alpha=0.0, z_form=0, z_columns=0):
         p = lam_default_params()
         p.nz = int(nz or n)
         p.kernel, p.width, p.oversample, p.shape = KERNELS[kernel], int(width), float(oversample), float(shape)
@@ -193,6 +194,7 @@ class Plan:
         p.t_min, p.device_bytes = float(t_min), int(device_bytes)
         p.plane_batch, p.theta_chunk = int(plane_batch), int(theta_chunk)
         p.pad_u, p.spectral_alpha = int(bool(pad_u)), float(spectral_alpha)
+        p.z_form, p.z_columns = int(z_form), int(z_columns)
         self.n, self.nz, self.h, self.w, self.ntheta = int(n), p.nz, int(h), int(w), len(theta)
         self.input = input
         self._plan = lam_create(n, h, w, theta, phi, p)

@@ -344,21 +344,22 @@ def test_host_pointers_pinned_and_pageable(pinned):
     plan.close()
 
 
-@pytest.mark.parametrize("lcb", [4, 3, 2])
-def test_x3_stage_tma_and_plain_kernels_agree(monkeypatch, lcb):
+@pytest.mark.parametrize("columns", [16, 8, 4])
+def test_x3_stage_tma_and_plain_kernels_agree(columns):
     """The x3 stage has two forms (k_zstage_tma: persistent blocks fed by TMA, the default below sigma*nz = 2048, and the
     plain k_zstage, used by long transforms and by the spilled schedule), each with 16, 8 or 4 columns per block (the
-    full-size configs use 16 / 8 / 4; the TMA form splits a cell's band over 1 / 2 / 4 lanes).  Same tables, same
-    arithmetic up to the order of the partial sums: both against the oracle, and against each other at fp32 rounding."""
+    full-size configs use 16 / 8 / 4; the TMA form splits a cell's band over 1 / 2 / 4 lanes), chosen here through
+    params.z_form / params.z_columns.  Same tables, same arithmetic up to the order of the partial sums: both against the
+    oracle, and against each other at fp32 rounding."""
     cfg = inputs.scaled(2, 256)
     d = inputs.projections(cfg)
     vols = {}
-    monkeypatch.setenv("LAM_TUNE_ZLCB", str(lcb))       # both read by lam_create
-    for mode in ("1", "0"):
-        monkeypatch.setenv("LAM_TUNE_ZTMA", mode)
-        vols[mode], _ = run_gpu(cfg, d)
-    monkeypatch.delenv("LAM_TUNE_ZTMA")
-    monkeypatch.delenv("LAM_TUNE_ZLCB")
+    for mode, form in (("1", 2), ("0", 1)):
+        plan = lam.Plan(cfg.n, cfg.h, cfg.w, d["theta"], cfg.phi, nz=cfg.nz, width=cfg.width, oversample=cfg.oversample,
+                        z_form=form, z_columns=columns)
+        vols[mode] = plan.backproject(d["proj"].cuda()).cpu().numpy()
+        plan.close()
+    lcb = columns.bit_length() - 1
     ref = O.fbp_gridded(geometry(cfg, d), d["proj"].numpy())
     for mode, v in vols.items():
         print("x3 stage", "tma" if mode == "1" else "plain", 1 << lcb, "columns:", tight(v, ref, f"x3 stage mode {mode}"))
