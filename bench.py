@@ -40,6 +40,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-full-config", type=int, default=-1,
+                    help="also run oracle path C in full on this config (0..2; minutes of host time) into all_configs[...].cpu_baseline")
     ap.add_argument("--cpu-angles", type=int, default=0, help="angles in the oracle's sample (0: auto)")
     return ap.parse_args()
 
@@ -110,6 +112,26 @@ def stage_model(cfg):
     }
 
 
+# SURVEY.md section 8(d) "Which roofline binds": ALGORITHMIC GB per step on the Hermitian-half 3-D grid (S3 there is the
+# whole pruned three-pass transform, S4 the deapodise pass; here the x3 pass lives in stage 4, so S3 + S4 are given as one
+# figure).  The factored method of Eq. 9 grids (h/2+1) planes of M^2 cells where the 3-D grid has sigma*nz/2: its own
+# work is what stage_model() counts; the survey's figure is printed beside it so both fractions are in the line.
+SURVEY_GB = {2: {"s1": 10.1, "s2": 13.6, "s3_s4": 22.5 + 2.1, "step": 48.4},
+             3: {"s1": 45.3, "s2": 98.9, "s3_s4": 180.0 + 17.2, "step": 342.0},
+             4: {"s1": 151.0, "s2": 650.0, "s3_s4": 1443.0 + 137.0, "step": 2382.0}}
+
+
+def survey_report(idx, stage, ms_step, hbm):
+    """Per-stage and whole-step HBM fractions on SURVEY.md 8(d)'s byte counts (None for configs it does not tabulate)."""
+    g = SURVEY_GB.get(idx)
+    if g is None:
+        return None
+    f = lambda gb, ms: round(gb / (ms * 1e-3) / hbm, 4) if ms > 0 else None
+    return {"algorithmic_GB_survey": g,
+            "hbm_frac_survey": {"s1": f(g["s1"], stage[0]), "s2": f(g["s2"], stage[1]), "s3_s4": f(g["s3_s4"], stage[2] + stage[3]),
+                                "step": f(g["step"], ms_step)}}
+
+
 def cpu_sample(cfg, nangles=None, slab=4, mult=3):
     """The oracle as it stands, path C (the double-precision gridded USFFT of PAPER.md:130-142: 3-D gridding with
     W^3 taps per sample, 3-D inverse FFT, deapodisation), on a BOUNDED sample of the config: the full detector and the
@@ -157,6 +179,24 @@ def cpu_sample(cfg, nangles=None, slab=4, mult=3):
                       f"{cfg.n}x{cfg.n} lateral grid, a slab of {slab} of {cfg.nz} x3-slices, {used[0]} and {used[1]} of "
                       f"{cfg.ntheta} angles: t_angle={t_angle:.3f}s, t_fix(slab)={t_fix:.2f}s; whole job = ntheta*t_angle + "
                       f"t_fix*{grow:.1f} (extrapolated)"}
+
+
+def cpu_full_path_c(idx, device="cpu"):
+    """Oracle path C IN FULL on one config (no sampling, no extrapolation): SURVEY.md 8(d) names it for configs[0]-[2]
+    (the fp64 fine grid of configs[2] is 34 GB).  Minutes of host time, so bench.py runs it only with --cpu-full-config."""
+    from oracle import lam_oracle as O
+    from paper_2401_11101_b200 import inputs
+    cfg = inputs.config(idx)
+    d = inputs.projections(cfg, device=device)
+    proj = d["proj"].cpu().contiguous().numpy()
+    g = O.Geometry(cfg.n, cfg.h, cfg.w, cfg.theta(), cfg.phi, nz=cfg.nz,
+                   dark=None if d["dark"] is None else d["dark"].cpu().numpy(), flat=None if d["flat"] is None else d["flat"].cpu().numpy())
+    del d
+    t0 = time.perf_counter()
+    O.fbp_gridded(g, proj, W=cfg.width, sigma=cfg.oversample)
+    dt = time.perf_counter() - t0
+    return {"value": float(f"{cfg.voxels / dt / 1e9:.6g}"), "unit": UNIT, "cores": O.threads(), "kind": "oracle",
+            "seconds": round(dt, 1), "sample": f"oracle path C in full on configs[{idx}] {cfg.name} (all {cfg.ntheta} angles, whole volume): measured, not extrapolated"}
 
 
 def max_over_ranks(ms, world, device):
@@ -295,21 +335,32 @@ def measure_next_rows(idx, reps=3):
 
     out = {"workload": f"{cfg.name}: volume {cfg.n}x{cfg.n}x{cfg.nz}, {cfg.ntheta} angles, detector {cfg.h}x{cfg.w} fp32"}
     t = timed(lambda: plan.forward(vol, proj), reps)
-    out["lam_forward"] = {"ms": round(t, 3), "GVoxel_per_s": round(cfg.voxels / t / 1e6, 3)}
+    # correctness beside the timing: <L f, d> = <f, L* d> on this very plan (L* = lam_backproject, filter none, whose
+    # columns the tests compare with the exact oracle at this size)
+    dd = torch.randn((cfg.ntheta, cfg.h, cfg.w), device="cuda")
+    ltd = plan.backproject(dd)
+    a, b = float((proj.double() * dd.double()).sum()), float((vol.double() * ltd.double()).sum())
+    out["lam_forward"] = {"ms": round(t, 3), "GVoxel_per_s": round(cfg.voxels / t / 1e6, 3),
+                          "adjoint_identity_rel": float(f"{abs(a - b) / float(proj.double().norm() * dd.double().norm()):.3e}")}
     centers = [cfg.w / 2 - 1.0, cfg.w / 2, cfg.w / 2 + 1.0]
     sl = torch.empty((3, cfg.n, cfg.n), device="cuda")
     t3 = timed(lambda: plan.backproject_slice(proj, cfg.nz // 2, centers, sl), 1)
     t1 = timed(lambda: plan.backproject_slice(proj, cfg.nz // 2, centers[:1], sl[:1]), 1)
-    out["lam_backproject_slice"] = {"ms_first_centre": round(t1, 3), "ms_per_further_centre": round((t3 - t1) / 2, 3)}
-    t_a = time.perf_counter()
-    plan.admm_tv(proj, 0.1, 1.0, 1, 2, vol)
-    torch.cuda.synchronize()
-    t2 = (time.perf_counter() - t_a) * 1e3
-    t_a = time.perf_counter()
-    plan.admm_tv(proj, 0.1, 1.0, 1, 4, vol)
-    torch.cuda.synchronize()
-    t4 = (time.perf_counter() - t_a) * 1e3
-    out["lam_admm_tv"] = {"ms_per_cg_step": round((t4 - t2) / 2, 3), "note": "one lam_forward + one lam_backproject + TV kernels and reductions per step"}
+    plan.backproject_slice(proj, cfg.nz // 2, None, sl[:1])
+    plan.backproject(proj, ltd)
+    ref = ltd[cfg.nz // 2]
+    out["lam_backproject_slice"] = {"ms_first_centre": round(t1, 3), "ms_per_further_centre": round((t3 - t1) / 2, 3),
+                                    "slice_vs_full_volume_rel_l2": float(f"{float((sl[0] - ref).norm() / ref.norm()):.3e}")}
+    del dd, ltd
+    # one CG step = one lam_forward + one lam_backproject + TV kernels and reductions: warm-up call first (it allocates
+    # the workspace), then the difference of a 4-step and a 2-step call, each timed with CUDA events
+    plan.admm_tv(proj, 0.1, 1.0, 1, 1, vol)
+    hist = []
+    t2 = timed(lambda: hist.append(plan.admm_tv(proj, 0.1, 1.0, 1, 2, vol)[1]), 1)
+    t4 = timed(lambda: hist.append(plan.admm_tv(proj, 0.1, 1.0, 1, 4, vol)[1]), 1)
+    out["lam_admm_tv"] = {"ms_per_cg_step": round((t4 - t2) / 2, 3), "ms_2_steps": round(t2, 3), "ms_4_steps": round(t4, 3),
+                          "gradF_norm_after_each_step": [float(f"{x:.4e}") for x in hist[-1]],
+                          "note": "one lam_forward + one lam_backproject + TV kernels and reductions per step"}
     plan.close()
     del vol, proj, sl
     torch.cuda.empty_cache()
@@ -391,6 +442,9 @@ def run_ours(args):
                     "ms_per_step_median": round(o["median_ms"], 3), "steps": k, "warmup": 3 if idx != 4 else 2,
                     "plan_ms": round(o["plan_ms"], 1), "stages": stage_report(c, o["stage"], hbm),
                     "copies_ms": round(o["stage"][4], 2), "overlap": o["overlap"], "plan": o["info"]}
+                sv = survey_report(idx, o["stage"], oms, hbm)
+                if sv:
+                    others[f"configs[{idx}]"].update(sv)
             except Exception as e:  # a config that does not fit this box must not void the headline line
                 others[f"configs[{idx}]"] = {"error": str(e)[:200]}
                 torch.cuda.empty_cache()
@@ -411,18 +465,25 @@ def run_ours(args):
     names = list(model.keys())
     stages = stage_report(cfg, stage, hbm)
     dom = max(range(4), key=lambda i: stage[i])
+    ach = model[names[dom]]["bytes"] / (stage[dom] * 1e-3) / 1e9
+    roof = {"kernel": "k_spread (+k_zero_tiles)" if names[dom] == "s2_gridding_xy" else names[dom], "stage": names[dom],
+            "bound": "hbm", "achieved": round(ach, 1), "peak": hbm, "unit": "GB/s", "frac": round(ach / hbm, 4),
+            "traffic": None, "peak_source": src}
     if names[dom] == "s2_gridding_xy":
-        # S2 is bound by instruction issue and the shared-memory pipe, not by HBM: reported against
-        # the fp32 FMA peak derived from unit counts and clocks, with its HBM fraction beside it in `stages`
-        peak = 148 * 128 * 2 * 1.965e9 / 1e12
-        ach = model[names[dom]]["flops"] / (stage[dom] * 1e-3) / 1e12
-        roof = {"kernel": "k_spread (+k_zero_tiles)", "stage": names[dom], "bound": "alu", "achieved": round(ach, 3),
-                "peak": round(peak, 2), "unit": "TFLOP/s", "frac": round(ach / peak, 4), "traffic": None,
-                "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 flop x 1.965 GHz"}
-    else:
-        ach = model[names[dom]]["bytes"] / (stage[dom] * 1e-3) / 1e9
-        roof = {"kernel": names[dom], "stage": names[dom], "bound": "hbm", "achieved": round(ach, 1), "peak": hbm,
-                "unit": "GB/s", "frac": round(ach / hbm, 4), "traffic": None, "peak_source": src}
+        # With the factored gridding of Eq. 9 (W^2 = 36 taps per sample instead of W^3 = 216) the fp32-ALU floor of S2
+        # (samples x 36 taps x 3 lane-instr / 3.72e13 per s) lies BELOW its HBM floor, so HBM is the binding roofline and
+        # `frac` is taken against it.  What the kernel actually saturates is the shared-memory (LSU) data pipe
+        # (DESIGN.md section 5); the ALU and LSU-pipe figures are kept here as context.
+        samples = model[names[dom]]["flops"] / (4 * cfg.width * cfg.width + 2 * cfg.width)
+        alu_peak = 148 * 128 * 2 * 1.965e9 / 1e12
+        alu_ach = model[names[dom]]["flops"] / (stage[dom] * 1e-3) / 1e12
+        lsu_floor_ms = samples * cfg.width * cfg.width * 16 / (148 * 128 * 1.965e9) * 1e3
+        roof["alu"] = {"achieved_TFLOPs": round(alu_ach, 3), "peak_TFLOPs": round(alu_peak, 2), "frac": round(alu_ach / alu_peak, 4),
+                       "floor_ms": round(samples * cfg.width * cfg.width * 3 / (148 * 128 * 1.965e9) * 1e3, 2),
+                       "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 flop x 1.965 GHz"}
+        roof["lsu_pipe"] = {"floor_ms": round(lsu_floor_ms, 2), "frac": round(lsu_floor_ms / stage[dom], 4),
+                            "note": "samples x W^2 taps x 16 B of shared-memory read-modify-write at 128 B/clk/SM"}
+        roof["hbm_floor_ms"] = round(model[names[dom]]["bytes"] / hbm / 1e6, 2)
     # traffic: dram bytes per launch of the dominant kernel from a committed ncu --set full capture, used only when that
     # capture was taken on THIS build and THIS launch shape (library version, config, plane batch); otherwise null
     try:
@@ -438,6 +499,10 @@ def run_ours(args):
     roof["share_of_step"] = round(stage[dom] / max(1e-9, sum(stage[:4])), 4)
     total_bytes = sum(m["bytes"] for m in model.values())
     roof["whole_step_hbm_frac"] = round(total_bytes / (ms_step * 1e-3) / 1e9 / hbm, 4)
+    roof["whole_step_algorithmic_GB"] = round(total_bytes / 1e9, 2)
+    sv = survey_report(args.config, stage, ms_step, hbm)
+    if sv:
+        roof.update(sv)
     out = {"metric": METRIC, "value": round(value, 4), "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": warmup, "ms_per_step": round(ms_step, 4), "ms_per_step_median": round(r["median_ms"], 4),
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -455,6 +520,9 @@ def run_ours(args):
         out["all_configs"] = others
     if next_rows:
         out["next_rows"] = next_rows
+    if 0 <= args.cpu_full_config <= 2:
+        torch.cuda.empty_cache()
+        out.setdefault("all_configs", {}).setdefault(f"configs[{args.cpu_full_config}]", {})["cpu_baseline"] = cpu_full_path_c(args.cpu_full_config, "cuda")
     if not args.no_cpu_baseline:
         cb = cpu_sample(cfg)
         out["cpu_baseline"] = {"value": float(f"{cb['value']:.6g}"), "unit": UNIT, "cores": cb["cores"], "kind": "oracle",
