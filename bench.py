@@ -488,7 +488,7 @@ def run_ours(args):
     # capture was taken on THIS build and THIS launch shape (library version, config, plane batch); otherwise null
     try:
         import csv
-        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "r02_traffic.csv"))):
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "r03_traffic.csv"))):
             if (int(row["config"]) == args.config and row["stage"] == names[dom] and row["lib_version"] == lam.lam_version()
                     and int(row["plane_batch"]) == r["info"]["plane_batch"]):
                 roof["traffic"] = float(row["dram_bytes_per_launch"])

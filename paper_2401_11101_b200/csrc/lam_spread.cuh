@@ -30,14 +30,7 @@
 
 namespace lam {
 
-#ifndef LAM_SW
-#define LAM_SW 1
-#endif
-#ifndef LAM_PIPE
-#define LAM_PIPE 0
-#endif
-constexpr int kSW = LAM_SW;        // warps per job = strips of 32 major-axis cells
-constexpr bool kPipe = LAM_PIPE;   // software-pipelined pair loop (more registers) or the plain one (more warps)
+constexpr int kSW = 1;             // warps per job: one warp owns one 32 x 32 tile (wider jobs were measured slower)
 constexpr int kTS = 32 * kSW;      // tile edge (fine-grid cells)
 constexpr int kJobRanges = 6;      // theta ranges per job
 constexpr int kJobMaxLines = 256;  // lines per job; a tile crossed by more lines is split over several jobs
@@ -153,6 +146,11 @@ __global__ void k_jobs(JobsArgs a) {
       for (int sx = -1; sx <= 1; ++sx) {
         if (!(mskx >> (sx + 1) & 1)) continue;
         const float ox = (float)(rho * cs.y - mx0 + (double)sx * g.M);
+        // cheap exact-side rejection (99 % of all (tile, theta) pairs miss): the grown box of clip_box lies inside the
+        // disc of radius sqrt(2) ((kTS - 1)/2 + W/2 + 0.02) around the tile centre; a line further away than that
+        // (+0.05 for the fp32 rounding of ox, oy at |coordinates| <= 1e4) cannot have a sample in it
+        constexpr float kHalf = 0.5f * (kTS - 1), kReach = 1.41421357f * (kHalf + 0.5f * W + 0.02f) + 0.05f;
+        if (fabsf((kHalf - ox) * s - (kHalf - oy) * c) > kReach) continue;
         int ka, kb;
         clip_box<W>(ox, oy, c, s, g.a1, g.w / 2, kTS, kTS, ka, kb);
         if (ka <= kb) { hx |= 1 << (sx + 1); hy |= 1 << (sy + 1); any = true; }
@@ -291,7 +289,7 @@ constexpr size_t spread_smem() {
 }
 
 template <int W>
-__global__ void __launch_bounds__(32 * kSW, kSW == 1 ? 20 : 6) k_spread(SpreadArgs a) {
+__global__ void __launch_bounds__(32 * kSW, 20) k_spread(SpreadArgs a) {
   extern __shared__ float2 smem[];
   float2* tile = smem;                                            // [kTS][kTS]: [minor][major]
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -443,8 +441,6 @@ __global__ void __launch_bounds__(32 * kSW, kSW == 1 ? 20 : 6) k_spread(SpreadAr
                 const int ls = max(is, seg), cnt = min(ie, seg + 31) - ls + 1;
                 const int NI = __reduce_max_sync(0xffffffffu, cnt);
                 if (NI <= 0) continue;
-                // software pipeline: the taps of pair i are loaded, the weights of pair i+1 are evaluated while those
-                // loads are in flight, then pair i is accumulated and stored
                 auto prep = [&](int i, float2& vw, float (&wm)[W], unsigned& addr, unsigned& rm) {
                   const int k = min(ls - seg + i, 31);
                   const float PM = fmaf((float)(ls + i), aM, PM0);
@@ -472,49 +468,20 @@ __global__ void __launch_bounds__(32 * kSW, kSW == 1 ? 20 : 6) k_spread(SpreadAr
                   addr = mycol_addr + (unsigned)(r0 * (kTS * 8));
                   rm = ok ? pk >> 8 : 0u;
                 };
-                if constexpr (kPipe) {
-                  float2 vw, nvw, c[W];
-                  float wm[W], nwm[W];
-                  unsigned addr, naddr, rm, nrm;
-                  prep(0, vw, wm, addr, rm);
+#pragma unroll 1
+                for (int i = 0; i < NI; ++i) {
+                  float2 vw, c[W];
+                  float wm[W];
+                  unsigned addr, rm;
+                  prep(i, vw, wm, addr, rm);
                   static_for<0, W>([&](auto J) {
                     if (rm >> J.value & 1u) c[J.value] = lds_f2<j_off(J.value)>(addr);
                   });
-                  for (int i = 0;;) {
-                    const bool last = i + 1 >= NI;
-                    if (!last) prep(i + 1, nvw, nwm, naddr, nrm);
 #pragma unroll
-                    for (int j = 0; j < W; ++j) c[j] = __ffma2_rn(vw, make_float2(wm[j], wm[j]), c[j]);
-                    static_for<0, W>([&](auto J) {
-                      if (rm >> J.value & 1u) sts_f2<j_off(J.value)>(addr, c[J.value]);
-                    });
-                    if (last) break;
-                    ++i;
-                    vw = nvw;
-#pragma unroll
-                    for (int j = 0; j < W; ++j) wm[j] = nwm[j];
-                    addr = naddr;
-                    rm = nrm;
-                    static_for<0, W>([&](auto J) {
-                      if (rm >> J.value & 1u) c[J.value] = lds_f2<j_off(J.value)>(addr);
-                    });
-                  }
-                } else {
-#pragma unroll 1
-                  for (int i = 0; i < NI; ++i) {
-                    float2 vw, c[W];
-                    float wm[W];
-                    unsigned addr, rm;
-                    prep(i, vw, wm, addr, rm);
-                    static_for<0, W>([&](auto J) {
-                      if (rm >> J.value & 1u) c[J.value] = lds_f2<j_off(J.value)>(addr);
-                    });
-#pragma unroll
-                    for (int j = 0; j < W; ++j) c[j] = __ffma2_rn(vw, make_float2(wm[j], wm[j]), c[j]);
-                    static_for<0, W>([&](auto J) {
-                      if (rm >> J.value & 1u) sts_f2<j_off(J.value)>(addr, c[J.value]);
-                    });
-                  }
+                  for (int j = 0; j < W; ++j) c[j] = __ffma2_rn(vw, make_float2(wm[j], wm[j]), c[j]);
+                  static_for<0, W>([&](auto J) {
+                    if (rm >> J.value & 1u) sts_f2<j_off(J.value)>(addr, c[J.value]);
+                  });
                 }
               }
               cur = nxt;
