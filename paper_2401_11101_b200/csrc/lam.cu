@@ -376,17 +376,21 @@ lam_status build_jobs(lam_plan* p) {
     p->job_off.assign(nb + 1, 0);
     p->multi_off.assign(nb + 1, 0);
     std::vector<unsigned> multi;
-    std::vector<unsigned> order;
+    std::vector<unsigned> order, bucket;
     long long tot = 0;
     const int nt = p->geom.nt;
     for (int b = 0; b < nb; ++b) {
       const size_t i0 = (size_t)b * PB * ntiles, i1 = (size_t)std::min(NP, (b + 1) * PB) * ntiles;
       p->job_off[b] = tot;
       p->multi_off[b] = (long long)multi.size();
+      // heaviest tiles first: a stable counting sort by descending line count (top bits of `lines`: image masks)
       order.resize(i1 - i0);
-      for (size_t i = 0; i < order.size(); ++i) order[i] = (unsigned)i;
-      std::stable_sort(order.begin(), order.end(),
-                       [&](unsigned x, unsigned y) { return (lines[i0 + x] & 0xffffffu) > (lines[i0 + y] & 0xffffffu); });  // top bits: image masks
+      unsigned kmax = 0;
+      for (size_t i = i0; i < i1; ++i) kmax = std::max(kmax, lines[i] & 0xffffffu);
+      bucket.assign((size_t)kmax + 2, 0);
+      for (size_t i = i0; i < i1; ++i) ++bucket[kmax - (lines[i] & 0xffffffu) + 1];
+      for (size_t b = 1; b < bucket.size(); ++b) bucket[b] += bucket[b - 1];
+      for (size_t i = i0; i < i1; ++i) order[bucket[kmax - (lines[i] & 0xffffffu)]++] = (unsigned)(i - i0);
       for (unsigned o : order) {
         const size_t i = i0 + o;
         offs[i] = (unsigned)tot;
